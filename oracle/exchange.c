@@ -1,0 +1,112 @@
+/* exchange.c -- CPU ORACLE (test infrastructure): per-cell implicit matter-radiation
+ * coupling, PAPER.md:198-265 (eq 26-43).  See qk_oracle.h for the role of this code.
+ *
+ * Readings: X1 eq 28 is taken as R = dt rho kappa_P c_hat (a_r T^4 - E_r)
+ * (the printed "4 pi B - c_hat E_r" is dimensionally inconsistent with eq 15-16 and with
+ * its own Jacobian eq 30, 32; 4 pi B = c a_r T^4 and the RSLA factor c_hat/c multiplies it).
+ * X2 C_v is the volumetric heat capacity dE_g/dT.  X5 converge-then-polish stop rule unless
+ * ORC_FLAG_NEWTON_LITERAL. */
+#include <math.h>
+#include <stdlib.h>
+#include "qk_oracle.h"
+
+#define NG ORC_NG
+
+/* T and C_v = dE_g/dT from the gas internal energy density */
+static void eos_T_Cv(const orc_grid *g, double rho, double Eg, double *T, double *Cv)
+{
+    if (g->eos == ORC_EOS_ALPHA_T3) {          /* eq 55: E_g = alpha T^4/4, C_v = alpha T^3 */
+        double t = sqrt(sqrt(4.0 * Eg / g->alpha));
+        *T = t; *Cv = g->alpha * (t * t * t);
+    } else {                                    /* ideal gas: E_g = rho kB/(mu mH) T/(gamma-1) */
+        double cv = rho * g->kB_mu / (g->gamma - 1.0);
+        *Cv = cv; *T = Eg / cv;
+    }
+}
+
+/* Updates (m, E, Er, F) of one cell over dt.  Returns 0 ok, 4 Newton failure, 5 bad state. */
+int orc_exchange_cell(const orc_grid *g, double dt, double rho, double m[3], double *E,
+                      double *Er, double F[3], double kP, double kR, int *iters)
+{
+    const double c = g->c, ch = g->c_hat, coc = c / ch;
+    const double S = g->S_src;
+    int rc = 0;
+    double msq0 = (m[0] * m[0] + m[1] * m[1]) + m[2] * m[2];
+    double Ekin0 = 0.5 * msq0 / rho;
+    double Eg0 = *E - Ekin0;
+    double Er0 = *Er;
+    double Etot = Eg0 + coc * (Er0 + S);        /* eq 38 */
+    double coef = dt * rho * kP * ch;           /* dt rho kappa_P c_hat */
+    double Eg = Eg0, Erad = Er0;
+    int it = 0, done = 0;
+    const int literal = (g->flags & ORC_FLAG_NEWTON_LITERAL) != 0;
+    while (it < g->newton_maxit) {
+        double T, Cv;
+        eos_T_Cv(g, rho, Eg, &T, &Cv);
+        double T2 = T * T;
+        double T4 = T2 * T2;
+        double R = coef * (g->a_rad * T4 - Erad);                 /* eq 28 (reading X1) */
+        double FG = (Eg - Eg0) + coc * R;                         /* eq 26 */
+        double FR = (Erad - Er0) - (R + S);                       /* eq 27 */
+        int conv = (fabs(FG / Etot) < g->newton_tol) && (fabs(coc * FR / Etot) < g->newton_tol); /* eq 36-37 */
+        if (conv && literal) { done = 1; break; }
+        double dRdEg = coef * (4.0 * g->a_rad * (T2 * T)) / Cv;   /* eq 33, dkappa/dT = 0 */
+        double dFGdEg = 1.0 + coc * dRdEg;                        /* eq 29 */
+        double dFGdEr = -(coc * coef);                            /* eq 30 */
+        double dFRdEg = -dRdEg;                                   /* eq 31 */
+        double dFRdEr = 1.0 + coef;                               /* eq 32 */
+        double eta = -dFRdEg / dFGdEg;
+        double dEr = -(FR + eta * FG) / (dFRdEr + eta * dFGdEr);  /* eq 34 */
+        double dEg = -(FG + dEr * dFGdEr) / dFGdEg;               /* eq 35 */
+        Erad = Erad + dEr;
+        Eg = Eg + dEg;
+        ++it;
+        if (conv) { done = 1; break; }
+    }
+    if (!done) rc = 4;
+    if (iters) *iters = it;
+    /* eq 39-41 with kappa_F ~ kappa_R */
+    double denom = 1.0 + rho * kR * ch * dt;
+    double F1[3], m1[3];
+    for (int i = 0; i < 3; ++i) F1[i] = F[i] / denom;
+    if (g->flags & ORC_FLAG_STATIC_MATTER) {                       /* drop all v/c terms */
+        *E = Eg + Ekin0;
+        *Er = Erad;
+    } else {
+        for (int i = 0; i < 3; ++i) m1[i] = m[i] - (F1[i] - F[i]) / (ch * c);
+        double msq1 = (m1[0] * m1[0] + m1[1] * m1[1]) + m1[2] * m1[2];
+        double dEkin = 0.5 * (msq1 - msq0) / rho;
+        *E = Eg + (Ekin0 + dEkin);                                 /* eq 42 */
+        *Er = Erad - (ch / c) * dEkin;                             /* eq 43 */
+        for (int i = 0; i < 3; ++i) m[i] = m1[i];
+    }
+    for (int i = 0; i < 3; ++i) F[i] = F1[i];
+    if (!(Eg > 0.0) || !(*Er > 0.0)) rc = rc ? rc : 5;
+    return rc;
+}
+
+int orc_exchange(orc_grid *g, double dt)
+{
+    const int nx = g->nx, ny = g->ny, nz = g->nz;
+    long long fail = 0, tot = 0, bad = 0; int mx = 0;
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                long long cidx = ((long long)(k + NG) * (ny + 2 * NG) + (j + NG)) * (nx + 2 * NG) + (i + NG);
+                double m[3] = { g->f[ORC_MX][cidx], g->f[ORC_MY][cidx], g->f[ORC_MZ][cidx] };
+                double F[3] = { g->f[ORC_FX][cidx], g->f[ORC_FY][cidx], g->f[ORC_FZ][cidx] };
+                double E = g->f[ORC_E][cidx], Er = g->f[ORC_ER][cidx];
+                int it = 0;
+                int r = orc_exchange_cell(g, dt, g->f[ORC_RHO][cidx], m, &E, &Er, F,
+                                          g->f[ORC_KP][cidx], g->f[ORC_KR][cidx], &it);
+                if (r == 4) ++fail;
+                if (r == 5) ++bad;
+                tot += it; if (it > mx) mx = it;
+                g->f[ORC_MX][cidx] = m[0]; g->f[ORC_MY][cidx] = m[1]; g->f[ORC_MZ][cidx] = m[2];
+                g->f[ORC_FX][cidx] = F[0]; g->f[ORC_FY][cidx] = F[1]; g->f[ORC_FZ][cidx] = F[2];
+                g->f[ORC_E][cidx] = E; g->f[ORC_ER][cidx] = Er;
+            }
+    g->newton_fail_cells = fail; g->newton_total_iters = tot; g->newton_max_iters = mx;
+    g->bad_state_cells = bad;
+    return fail ? 4 : (bad ? 5 : 0);
+}

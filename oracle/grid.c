@@ -1,0 +1,191 @@
+/* grid.c -- CPU ORACLE (test infrastructure): storage, ghost fill, CFL, step drivers.
+ * See qk_oracle.h for the role of this code.  Citations: /root/reference/PAPER.md. */
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#include "qk_oracle.h"
+
+static long long sx(const orc_grid *g) { (void)g; return 1; }
+static long long sy(const orc_grid *g) { return (long long)(g->nx + 2 * ORC_NG); }
+static long long sz(const orc_grid *g) { return (long long)(g->nx + 2 * ORC_NG) * (g->ny + 2 * ORC_NG); }
+
+long long orc_ncells_total(const orc_grid *g)
+{
+    return (long long)(g->nx + 2 * ORC_NG) * (g->ny + 2 * ORC_NG) * (g->nz + 2 * ORC_NG);
+}
+
+/* index of cell (i,j,k), interior 0..n-1, ghosts -4..-1 and n..n+3 */
+static long long idx(const orc_grid *g, int i, int j, int k)
+{
+    return ((long long)(k + ORC_NG) * (g->ny + 2 * ORC_NG) + (j + ORC_NG)) * (g->nx + 2 * ORC_NG) + (i + ORC_NG);
+}
+
+orc_grid *orc_create(int nx, int ny, int nz, double dx, double gamma, double c_hat, double c, int bc)
+{
+    orc_grid *g = (orc_grid *)calloc(1, sizeof(orc_grid));
+    if (!g) return NULL;
+    g->nx = nx; g->ny = ny; g->nz = nz;
+    g->dx = dx; g->gamma = gamma; g->c_hat = c_hat; g->c = c; g->bc = bc;
+    g->a_rad = 1.0; g->kB_mu = 1.0;
+    g->cfl = 0.3; g->newton_tol = 1e-10; g->newton_maxit = 400; g->nsub_max = 10;
+    g->flags = ORC_FLAG_TAU_CORR;
+    g->eos = ORC_EOS_IDEAL; g->alpha = 0.0; g->S_src = 0.0;
+    long long n = orc_ncells_total(g);
+    for (int f = 0; f < ORC_NFIELDS; ++f) {
+        g->f[f] = (double *)calloc((size_t)n, sizeof(double));
+        if (!g->f[f]) { orc_destroy(g); return NULL; }
+    }
+    return g;
+}
+
+void orc_destroy(orc_grid *g)
+{
+    if (!g) return;
+    for (int f = 0; f < ORC_NFIELDS; ++f) free(g->f[f]);
+    free(g);
+}
+
+void orc_set_constants(orc_grid *g, double a_rad, double kB_mu) { g->a_rad = a_rad; g->kB_mu = kB_mu; }
+
+void orc_set_params(orc_grid *g, double cfl, double newton_tol, int newton_maxit, int nsub_max, unsigned flags)
+{
+    g->cfl = cfl; g->newton_tol = newton_tol; g->newton_maxit = newton_maxit;
+    g->nsub_max = nsub_max; g->flags = flags;
+}
+
+void orc_set_eos(orc_grid *g, int eos, double alpha) { g->eos = eos; g->alpha = alpha; }
+
+void orc_set_field(orc_grid *g, int field, const double *interior)
+{
+    for (int k = 0; k < g->nz; ++k)
+        for (int j = 0; j < g->ny; ++j)
+            for (int i = 0; i < g->nx; ++i)
+                g->f[field][idx(g, i, j, k)] = interior[((long long)k * g->ny + j) * g->nx + i];
+}
+
+void orc_get_field(const orc_grid *g, int field, double *interior)
+{
+    for (int k = 0; k < g->nz; ++k)
+        for (int j = 0; j < g->ny; ++j)
+            for (int i = 0; i < g->nx; ++i)
+                interior[((long long)k * g->ny + j) * g->nx + i] = g->f[field][idx(g, i, j, k)];
+}
+
+void orc_get_raw(const orc_grid *g, int field, double *with_ghosts)
+{
+    memcpy(with_ghosts, g->f[field], (size_t)orc_ncells_total(g) * sizeof(double));
+}
+
+void orc_set_raw(orc_grid *g, int field, const double *with_ghosts)
+{
+    memcpy(g->f[field], with_ghosts, (size_t)orc_ncells_total(g) * sizeof(double));
+}
+
+void orc_get_info(const orc_grid *g, long long *out7)
+{
+    out7[0] = g->last_nsub; out7[1] = g->newton_fail_cells; out7[2] = g->newton_max_iters;
+    out7[3] = g->newton_total_iters; out7[4] = g->bad_state_cells; out7[5] = g->fallback_states;
+    out7[6] = g->guard_faces;
+}
+
+/* source index along one axis for a ghost index (PAPER.md:293,572 periodic; 464 outflow).
+ * Outflow is read as zero-gradient: copy of the nearest interior cell (H15). */
+static int src_index(int i, int n, int bc)
+{
+    if (i >= 0 && i < n) return i;
+    if (bc == ORC_BC_PERIODIC) { int m = i % n; if (m < 0) m += n; return m; }
+    return i < 0 ? 0 : n - 1;
+}
+
+static void fill_one(orc_grid *g, double *a)
+{
+    /* every ghost cell (faces, edges, corners) <- the interior cell its three axis
+     * indices map to; equivalent to filling x, then y, then z in sequence. */
+    for (int k = -ORC_NG; k < g->nz + ORC_NG; ++k) {
+        int ks = src_index(k, g->nz, g->bc);
+        for (int j = -ORC_NG; j < g->ny + ORC_NG; ++j) {
+            int js = src_index(j, g->ny, g->bc);
+            for (int i = -ORC_NG; i < g->nx + ORC_NG; ++i) {
+                int is = src_index(i, g->nx, g->bc);
+                if (is == i && js == j && ks == k) continue;
+                a[idx(g, i, j, k)] = a[idx(g, is, js, ks)];
+            }
+        }
+    }
+}
+
+void orc_fill_field(orc_grid *g, int field) { fill_one(g, g->f[field]); }
+
+void orc_fill_boundary(orc_grid *g, int which)
+{
+    if (which & ORC_FILL_HYDRO) for (int f = ORC_RHO; f <= ORC_E; ++f) fill_one(g, g->f[f]);
+    if (which & ORC_FILL_RAD)   for (int f = ORC_ER; f <= ORC_FZ; ++f) fill_one(g, g->f[f]);
+    if (which & 4)              for (int f = ORC_KP; f <= ORC_KR; ++f) fill_one(g, g->f[f]);
+}
+
+/* eq 21: dt = CFL dx / max(|v| + c_s), |v| the vector magnitude
+ * (PAPER.md:142).  If c_hat > 0 the result is also limited so that the number of
+ * radiation substeps stays <= N_sub,max: dt <= nsub_max CFL dx / c_hat. */
+double orc_cfl_dt(orc_grid *g)
+{
+    double smax = 0.0;
+    long long bad = 0;
+    for (int k = 0; k < g->nz; ++k)
+        for (int j = 0; j < g->ny; ++j)
+            for (int i = 0; i < g->nx; ++i) {
+                long long c = idx(g, i, j, k);
+                double U[5] = { g->f[ORC_RHO][c], g->f[ORC_MX][c], g->f[ORC_MY][c], g->f[ORC_MZ][c], g->f[ORC_E][c] };
+                double W[5];
+                orc_cons_to_prim(g->gamma, U, W);
+                if (!(W[0] > 0.0) || !(W[4] > 0.0)) { ++bad; continue; }
+                double vmag = sqrt((W[1] * W[1] + W[2] * W[2]) + W[3] * W[3]);
+                double cs = sqrt(g->gamma * W[4] / W[0]);
+                double s = vmag + cs;
+                if (s > smax) smax = s;
+            }
+    g->bad_state_cells = bad;
+    if (bad) return NAN;
+    double dt = g->cfl * g->dx / smax;
+    if (g->c_hat > 0.0) {
+        double dtr = (double)g->nsub_max * (g->cfl * g->dx / g->c_hat);
+        if (dtr < dt) dt = dtr;
+    }
+    return dt;
+}
+
+/* number of radiation substeps for a hydro step dt */
+int orc_nsub_for(const orc_grid *g, double dt)
+{
+    double ratio = dt * g->c_hat / (g->cfl * g->dx);
+    int n = (int)ceil(ratio * (1.0 - 1e-12));
+    return n < 1 ? 1 : n;
+}
+
+int orc_rad_step(orc_grid *g, double dt)
+{
+    int rc = orc_rad_transport(g, dt);
+    if (rc) return rc;
+    return orc_exchange(g, dt);                 /* once per subcycle */
+}
+
+/* operator-split cycle: hydro, then N_sub x (transport, exchange) */
+int orc_rhd_step(orc_grid *g, double dt)
+{
+    int nsub = orc_nsub_for(g, dt);
+    if (nsub > g->nsub_max) return 1;
+    int rc = orc_hydro_step(g, dt);
+    if (rc) return rc;
+    double dts = dt / (double)nsub;
+    long long fail = 0, tot = 0, fb = 0, gf = 0; int mx = 0;
+    for (int s = 0; s < nsub; ++s) {
+        rc = orc_rad_step(g, dts);
+        fail += g->newton_fail_cells; tot += g->newton_total_iters;
+        fb += g->fallback_states; gf += g->guard_faces;
+        if (g->newton_max_iters > mx) mx = g->newton_max_iters;
+        if (rc) break;
+    }
+    g->last_nsub = nsub; g->newton_fail_cells = fail; g->newton_total_iters = tot;
+    g->newton_max_iters = mx; g->fallback_states = fb; g->guard_faces = gf;
+    (void)sx; (void)sy; (void)sz;
+    return rc;
+}
