@@ -170,6 +170,7 @@ def test_sod_against_exact_solution():
     assert 1.6 < errs[0] / errs[1] < 2.6 and 1.6 < errs[1] / errs[2] < 2.6, errs
 
 
+@pytest.mark.slow
 def test_strong_shock_tube_error_scale():
     """PAPER.md:313-315: (rho,p) = (10,100)|(1,1), 1000 cells on [0,5], x0=2, t=0.4, CFL 0.1;
     relative rms-of-L1 error printed as 1.12e-3 (gamma not printed; 1.4 assumed: weak pin, ~1e-3)."""
