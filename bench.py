@@ -1,0 +1,389 @@
+#!/usr/bin/env python
+"""bench.py -- cell-updates/s of the QUOKKA cell update on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--size n]
+
+One "step" = one pass of the hot path over the box: qk_cfl_dt (eq 21) + qk_hydro_step for the
+headline hydro workload (BASELINE.json configs[1], 256^3 Mach-2 turbulence), and qk_cfl_dt +
+qk_rhd_step (hydro, N_sub x (radiation transport, exchange)) for the RHD workload
+(configs[3], 256^3), reported in the same JSON line under "rhd".  Inputs are the seeded
+synthetic generators of paper_2110_01792_b200.inputs.
+
+`value` is timed with CUDA events on the launching stream with the state resident in HBM;
+`e2e` is the same step through the C ABI with HOST buffers: every step copies the five
+conserved fields host->device from pinned memory (qk_set_state), advances, and copies them
+back (qk_get_state), all inside the timed region.  Working set per step (5 x 147 MB read,
+plus stage buffers) is several times the 126 MB L2, so no explicit flush is needed.
+
+--impl reference times the CPU oracle (oracle/, plain C, single thread) on a bounded sample of
+the same workload; it is a deliberately slow baseline.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "hydro_cell_updates_per_s"
+UNIT = "cell-updates/s"
+# algorithmic fp64 operations per cell per RK stage (counted from the
+# formulas of section 3: one evaluation of every quantity per cell / face, typical branches)
+OPS_HYDRO_STAGE = 1468.0
+OPS_RAD_STAGE = 1310.0
+BYTES_EXCHANGE = 152.0
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+# ---------------------------------------------------------------------------------------------
+# clocks during the timed region (B200_PROFILING.md recipe)
+# ---------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.idx = gpu_index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(["nvidia-smi", "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(self.idx)],
+                                         stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return None
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        try:
+            for line in open(self.path):
+                p = [x.strip() for x in line.split(",")]
+                if len(p) < 9:
+                    continue
+                try:
+                    sm.append(float(p[1])); mx.append(float(p[2]))
+                except ValueError:
+                    continue
+                for n, v in zip(names, p[5:9]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            os.unlink(self.path)
+        except Exception:
+            pass
+        if not sm:
+            return None
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+# ---------------------------------------------------------------------------------------------
+# the CPU oracle on a bounded sample (cpu_baseline leg and --impl reference)
+# ---------------------------------------------------------------------------------------------
+def oracle_sample(kind, n, steps, seed_shift=0):
+    """Time `steps` oracle steps of the workload generator at n^3.  Returns (updates/s, seconds)."""
+    import oracle as O
+    from paper_2110_01792_b200 import inputs as I
+    params, fields = (I.config2(n=n, seed=1002 + seed_shift) if kind == "hydro"
+                      else I.config4(n=n, seed=1004 + seed_shift))
+    g = O.Grid(params["nx"], params["ny"], params["nz"], params["dx"], params["gamma"],
+               c_hat=params.get("c_hat", 0.0), c=params.get("c", 0.0), bc=params["bc"])
+    if "a_rad" in params:
+        g.set_constants(params["a_rad"], params["kB_mu"])
+    g.set_params(cfl=params["cfl"], flags=params["flags"])
+    g.set_all(fields)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        dt = g.cfl_dt()
+        rc = g.hydro_step(dt) if kind == "hydro" else g.rhd_step(dt)
+        assert rc == 0, rc
+    sec = time.perf_counter() - t0
+    g.close()
+    return n ** 3 * steps / sec, sec
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    n = args.ref_size
+    # W warm-up "steps" and K timed ones, each one oracle step on the n^3 sample
+    import oracle as O
+    from paper_2110_01792_b200 import inputs as I
+    params, fields = I.config2(n=n)
+    g = O.Grid(n, n, n, params["dx"], params["gamma"], bc=params["bc"])
+    g.set_params(cfl=params["cfl"], flags=params["flags"])
+    g.set_all(fields)
+    for _ in range(args.warmup):
+        g.hydro_step(g.cfl_dt())
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        assert g.hydro_step(g.cfl_dt()) == 0
+    sec = time.perf_counter() - t0
+    g.close()
+    value = n ** 3 * args.steps / sec
+    sample = "oracle (plain C, -O2 -ffp-contract=off, 1 thread) on a %d^3 box of the config2 generator, %d steps" % (
+        n, args.steps)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec / args.steps * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "BASELINE.json configs[1] generator (hydro, Mach-2 turbulence, periodic, "
+                                   "gamma=5/3, CFL 0.3), bounded sample %d^3" % n},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ---------------------------------------------------------------------------------------------
+# the CUDA path
+# ---------------------------------------------------------------------------------------------
+def time_steps(torch, ctx, kind, nsteps, barrier):
+    """nsteps x (qk_cfl_dt + step) bracketed by barrier + synchronize, timed with CUDA events on the
+    stream the kernels are launched on.  Returns milliseconds."""
+    stream = torch.cuda.current_stream()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    torch.cuda.synchronize()
+    e0.record(stream)
+    for _ in range(nsteps):
+        dt = ctx.qk_cfl_dt()
+        if kind == "hydro":
+            ctx.qk_hydro_step(dt)
+        else:
+            ctx.qk_rhd_step(dt)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    barrier()
+    return e0.elapsed_time(e1)
+
+
+def time_steps_e2e(torch, ctx, kind, nsteps, host_in, host_out, barrier):
+    """Same step through the C ABI with HOST (pinned) buffers: H2D of the evolving fields, step,
+    D2H of the result, every step, inside the timed region."""
+    stream = torch.cuda.current_stream()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    nf = len(host_in)
+    barrier()
+    torch.cuda.synchronize()
+    e0.record(stream)
+    for _ in range(nsteps):
+        for f in range(nf):
+            ctx.qk_set_state(f, host_in[f])
+        dt = ctx.qk_cfl_dt()
+        if kind == "hydro":
+            ctx.qk_hydro_step(dt)
+        else:
+            ctx.qk_rhd_step(dt)
+        for f in range(nf):
+            ctx.qk_get_state(f, host_out[f])
+        host_in, host_out = host_out, host_in      # next step starts from this step's result
+    e1.record(stream)
+    torch.cuda.synchronize()
+    barrier()
+    return e0.elapsed_time(e1)
+
+
+def run_workload(torch, B, I, kind, n, steps, warmup, rank, world, barrier, allmax, sampler=None):
+    t0 = time.time()
+    params, fields = (I.config2(n=n, seed=1002 + rank) if kind == "hydro" else I.config4(n=n, seed=1004 + rank))
+    log("[rank %d] %s %d^3 inputs generated in %.1f s" % (rank, kind, n, time.time() - t0))
+    nf = 5 if kind == "hydro" else 9
+    cells = n ** 3
+    out = {}
+    with B.from_params(params, fields) as ctx:
+        for _ in range(warmup):
+            dt = ctx.qk_cfl_dt()
+            ctx.qk_hydro_step(dt) if kind == "hydro" else ctx.qk_rhd_step(dt)
+        ctx.set_all(fields)                        # timed steps are steps 1..K of the config
+        torch.cuda.synchronize()
+        l0 = ctx.qk_launch_count()
+        ctx.qk_set_profiling(True)
+        if sampler:
+            sampler.start()
+        ms = time_steps(torch, ctx, kind, steps, barrier)
+        clocks = sampler.stop() if sampler else None
+        ktimes = ctx.qk_kernel_times()
+        ctx.qk_set_profiling(False)
+        launches = ctx.qk_launch_count() - l0
+        info = ctx.qk_last_info()
+        ms = allmax(ms)
+        out.update(ms=ms, value=world * cells * steps / (ms * 1e-3), launches=launches, kernel_ms=ktimes,
+                   clocks=clocks, info=info)
+        # end to end with host buffers
+        host_a = [torch.from_numpy(np.ascontiguousarray(fields[I.FIELDS[f]])).pin_memory() for f in range(nf)]
+        host_b = [torch.empty_like(t).pin_memory() for t in host_a]
+        e2e_steps = max(1, min(steps, 5))
+        time_steps_e2e(torch, ctx, kind, 1, [t.clone().pin_memory() for t in host_a], host_b, barrier)  # warm
+        ms_e = allmax(time_steps_e2e(torch, ctx, kind, e2e_steps, host_a, host_b, barrier))
+        out["e2e"] = {"value": world * cells * e2e_steps / (ms_e * 1e-3), "unit": UNIT,
+                      "h2d_bytes_per_step": nf * cells * 8, "d2h_bytes_per_step": nf * cells * 8,
+                      "ms_per_step": ms_e / e2e_steps, "steps": e2e_steps}
+    return out
+
+
+def roofline_alu(kernel_ms, names, ops_per_cell_per_launch, cells, peak_ops, peak_note):
+    """Dominant ALU-bound kernel: algorithmic fp64 ops per launch / mean launch duration."""
+    for nm in names:
+        if nm in kernel_ms:
+            tot, cnt = kernel_ms[nm]
+            mean_ms = tot / cnt
+            achieved = ops_per_cell_per_launch * cells / (mean_ms * 1e-3) / 1e12
+            return {"bound": "alu", "kernel": nm, "achieved": achieved, "peak": peak_ops / 1e12,
+                    "unit": "TFLOP/s", "frac": achieved / (peak_ops / 1e12), "traffic": None,
+                    "launch_ms": mean_ms, "launches": cnt, "peak_source": peak_note,
+                    "ops_per_cell_per_launch": ops_per_cell_per_launch}
+    return None
+
+
+def run_ours(args):
+    import torch
+    from paper_2110_01792_b200 import binding as B
+    from paper_2110_01792_b200 import inputs as I
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the library has no CPU path)")
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+
+    def allmax(x):
+        if dist is None:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    B.lib()     # fails loudly if libqk.so is absent
+    n = args.size
+    cells = n ** 3
+    # roofline denominators: measured fp64 pipe rate (DMUL+DADD mix, -fmad=false) and HBM copy
+    peak_ops = B.qk_fp64_probe(0, 4000)
+    peak_fma = B.qk_fp64_probe(1, 4000)
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm = float(peaks.get("hbm_gbs", 6650.0))
+    hbm_note = "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    hyd = run_workload(torch, B, I, "hydro", n, args.steps, args.warmup, rank, world, barrier, allmax, sampler)
+    rhd = None
+    if not args.no_rhd:
+        rhd_steps = max(1, min(args.steps, args.rhd_steps))
+        rhd = run_workload(torch, B, I, "rhd", n, rhd_steps, min(args.warmup, 3), rank, world, barrier, allmax)
+        rhd["steps"] = rhd_steps
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    peak_note = "qk_fp64_probe: measured DMUL+DADD lane-ops/s on this GPU (DFMA probe: %.2f T/s)" % (peak_fma / 1e12)
+    roof = roofline_alu(hyd["kernel_ms"], ["hydro_stage", "hydro_flux"],
+                        OPS_HYDRO_STAGE if "hydro_stage" in hyd["kernel_ms"] else OPS_HYDRO_STAGE / 3.0,
+                        cells, peak_ops, peak_note)
+    line = {
+        "metric": METRIC, "value": hyd["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": hyd["ms"] / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "BASELINE.json configs[1]: pure hydro %d^3, periodic, gamma=5/3, log-normal density, "
+                               "k^-2 velocity field at rms Mach 2, CFL 0.3, qk_cfl_dt + qk_hydro_step per step" % n,
+                   "cells": cells, "l2": "inputs larger than L2 (5 x %.0f MB per stage)" % (cells * 8 / 1e6),
+                   "parallelism": "1 box per GPU, no halo exchange (replicas)" if world > 1 else "1 box on 1 GPU"},
+        "e2e": hyd["e2e"], "gpu_launches": hyd["launches"], "clocks": hyd["clocks"],
+        "roofline": roof,
+        "kernel_ms": {k: {"total_ms": v[0], "groups": v[1]} for k, v in hyd["kernel_ms"].items()},
+        "peaks": {"fp64_dmul_dadd_lane_ops_per_s": peak_ops, "fp64_dfma_lane_ops_per_s": peak_fma,
+                  "hbm_gbs": hbm, "hbm_source": hbm_note},
+    }
+    if rhd is not None:
+        ex = rhd["kernel_ms"].get("exchange")
+        rroof = roofline_alu(rhd["kernel_ms"], ["rad_stage", "rad_flux"],
+                             OPS_RAD_STAGE if "rad_stage" in rhd["kernel_ms"] else OPS_RAD_STAGE / 3.0,
+                             cells, peak_ops, peak_note)
+        exroof = None
+        if ex:
+            ach = BYTES_EXCHANGE * cells / (ex[0] / ex[1] * 1e-3) / 1e9
+            exroof = {"bound": "hbm", "kernel": "exchange", "achieved": ach, "peak": hbm, "unit": "GB/s",
+                      "frac": ach / hbm, "traffic": None, "launch_ms": ex[0] / ex[1], "peak_source": hbm_note}
+        line["rhd"] = {
+            "metric": "rhd_cell_updates_per_s", "value": rhd["value"], "unit": UNIT, "steps": rhd["steps"],
+            "ms_per_step": rhd["ms"] / rhd["steps"], "nsub": rhd["info"]["nsub"],
+            "config": {"workload": "BASELINE.json configs[3]: coupled RHD %d^3, periodic, c_hat/c=0.01, "
+                                   "qk_cfl_dt + qk_rhd_step per step" % n},
+            "e2e": rhd["e2e"], "gpu_launches": rhd["launches"],
+            "roofline_rad": rroof, "roofline_exchange": exroof,
+            "kernel_ms": {k: {"total_ms": v[0], "groups": v[1]} for k, v in rhd["kernel_ms"].items()},
+            "newton_mean_iters": rhd["info"]["newton_total_iters"] / max(1, cells * rhd["info"]["nsub"]),
+        }
+    if world == 1 and not args.no_cpu_baseline:
+        v, sec = oracle_sample("hydro", args.ref_size, 2)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                "sample": "oracle (plain C, 1 thread) on a %d^3 box of the config2 generator, 2 steps, "
+                                          "%.1f s" % (args.ref_size, sec)}
+        if rhd is not None:
+            v2, sec2 = oracle_sample("rhd", max(16, args.ref_size * 3 // 4), 2)
+            line["rhd"]["cpu_baseline"] = {"value": v2, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                           "sample": "oracle on a %d^3 box of the config4 generator, 2 steps, %.1f s"
+                                                     % (max(16, args.ref_size * 3 // 4), sec2)}
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--size", type=int, default=256, help="box edge (BASELINE metric: 256)")
+    ap.add_argument("--rhd-steps", type=int, default=10)
+    ap.add_argument("--ref-size", type=int, default=128, help="edge of the oracle's bounded sample")
+    ap.add_argument("--no-rhd", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

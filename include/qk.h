@@ -1,0 +1,170 @@
+/* qk.h -- C ABI of the B200-native per-timestep uniform-grid cell update of the QUOKKA
+ * method (Wibking & Krumholz, arXiv:2110.01792).  Citations are /root/reference/PAPER.md
+ * line numbers ("PAPER.md:<line>") and DESIGN.md readings (H*, R*, X*).
+ *
+ * One context = one uniform box of nx*ny*nz cells with QK_NG ghost zones per side on one
+ * GPU, fp64, structure-of-arrays.  Every field is a dense array of
+ * (nz+2*QK_NG)*(ny+2*QK_NG)*(nx+2*QK_NG) doubles, x fastest; interior cell (i,j,k),
+ * 0-based, sits at ((k+QK_NG)*(ny+2*QK_NG) + (j+QK_NG))*(nx+2*QK_NG) + (i+QK_NG).
+ *
+ * All step functions run hand-written sm_100a CUDA kernels; there is no CPU fallback.
+ * They are asynchronous on the context's stream and return QK_OK once enqueued (or the
+ * CUDA launch error).  State errors found on the device (non-positive density, pressure
+ * or radiation energy; Newton failure) are counted there and surfaced by qk_last_info,
+ * which synchronises.  No function calls exit(); no global state; contexts are independent.
+ *
+ * Pointer arguments named `interior`/`with_ghosts` may be HOST or DEVICE pointers (the
+ * library asks the CUDA runtime which); set/get copy and never alias the caller's array.
+ */
+#ifndef QK_H
+#define QK_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define QK_NG 4   /* ghost zones per side: PPM needs 3, multidimensional flattening 4 (H6) */
+
+typedef struct qk_ctx qk_ctx;   /* opaque; owns layout, stage buffers, device counters */
+
+enum { QK_OK = 0, QK_EINVAL = 1, QK_ENOMEM = 2, QK_ECUDA = 3,
+       QK_ENEWTON = 4,   /* >=1 cell hit the Newton iteration cap              */
+       QK_ESTATE = 5 };  /* rho<=0, P<=0, E_g<=0 or E_r<=0 met (PAPER.md:438 needs E_r>0)      */
+
+enum { QK_BC_PERIODIC = 0,
+       QK_BC_OUTFLOW = 1 };  /* PAPER.md:464; zero-gradient copy of the nearest interior cell (H15) */
+
+/* field ids: conserved hydro U=(rho, rho v, E), radiation moments
+ * (E_r, F_r) (eq 11-12), Planck- and Rosseland-type opacities per cell
+ * (kappa_E~kappa_P, kappa_F~kappa_R), static during a step. */
+enum { QK_RHO = 0, QK_MX, QK_MY, QK_MZ, QK_E, QK_ER, QK_FX, QK_FY, QK_FZ, QK_KAPPA_P, QK_KAPPA_R,
+       QK_NFIELDS };
+
+enum { QK_FLAG_TAU_CORR = 1,        /* guarded optical-depth correction of the E_r HLL flux (R6) */
+       QK_FLAG_STATIC_MATTER = 2,   /* exchange skips eq 41-43: gas held at rest (X11)            */
+       QK_FLAG_NEWTON_LITERAL = 4 };/* literal stop rule of PAPER.md:237 instead of converge-then-polish (X5)   */
+
+enum { QK_FILL_HYDRO = 1, QK_FILL_RAD = 2, QK_FILL_OPACITY = 4, QK_FILL_ALL = 7 };
+
+/* Counters of the most recent step call (qk_hydro_step / qk_rad_step / qk_rhd_step / qk_exchange
+ * / qk_rad_transport), summed over the substeps of a qk_rhd_step. */
+typedef struct qk_info {
+    int       nsub;               /* radiation substeps taken by the last qk_rhd_step */
+    int       newton_max_iters;   /* largest Newton iteration count in any cell                      */
+    long long newton_fail_cells;  /* cells that reached newton_maxit without converging              */
+    long long newton_total_iters; /* sum of iteration counts over cells                               */
+    long long bad_state_cells;    /* cells flagged QK_ESTATE                                           */
+    long long fallback_states;    /* radiation face states reverted to first order     */
+    long long guard_faces;        /* faces where the tau correction was disabled       */
+    int       status;             /* QK_OK, QK_ENEWTON or QK_ESTATE                                   */
+} qk_info;
+
+/* Create a context for an nx*ny*nz box (each >= 1), cell size dx, adiabatic index gamma,
+ * reduced and physical speeds of light c_hat, c (eq 13-17; pass 0,0 for pure
+ * hydro) and boundary QK_BC_*.  Selects the current CUDA device.  Device memory for the
+ * state is allocated here with cudaMalloc unless `qk_bind_storage` supplies it before
+ * first use (allocation is deferred to first use).  Defaults: a_rad = 1, k_B/(mu m_H) = 1,
+ * CFL 0.3, Newton tolerance 1e-10, 400 iterations, N_sub,max 10,
+ * flags = QK_FLAG_TAU_CORR.  Returns QK_EINVAL / QK_ENOMEM / QK_ECUDA on failure. */
+int qk_init(int nx, int ny, int nz, double dx, double gamma, double c_hat, double c, int boundary,
+            qk_ctx **out);
+
+/* Destroy a context; frees device memory the library allocated (never bound storage). */
+int qk_free(qk_ctx *ctx);
+
+/* Bytes of device memory one context needs (11 state fields, 5 RK stage fields, the
+ * flattening coefficient, counters), for callers that own the allocation (torch.empty). */
+size_t qk_state_bytes(int nx, int ny, int nz);
+
+/* Use caller-owned DEVICE memory (>= qk_state_bytes, 256-byte aligned) instead of
+ * cudaMalloc.  Must precede the first set/get/step call.  The caller keeps ownership. */
+int qk_bind_storage(qk_ctx *ctx, void *dev_ptr, size_t bytes);
+
+/* cudaStream_t (as void*) all later work of this context is enqueued on; NULL = default. */
+int qk_set_stream(qk_ctx *ctx, void *cuda_stream);
+
+/* radiation constant a_r and k_B/(mu m_H) of the ideal-gas temperature
+ * T = (gamma-1) E_g / (rho k_B/(mu m_H)) (X2). */
+int qk_set_constants(qk_ctx *ctx, double a_rad, double kB_over_mu_mH);
+
+/* CFL number C0/D of eq 21, Newton tolerance and iteration cap,
+ * N_sub,max and QK_FLAG_* bits. */
+int qk_set_params(qk_ctx *ctx, double cfl, double newton_tol, int newton_maxit, int nsub_max,
+                  unsigned flags);
+
+/* Copy one field's interior, nz*ny*nx doubles x fastest (host or device), into / out of the
+ * state.  qk_get_state synchronises the stream before returning. */
+int qk_set_state(qk_ctx *ctx, int field, const double *interior);
+int qk_get_state(qk_ctx *ctx, int field, double *interior);
+
+/* Same with the ghost zones: (nz+8)(ny+8)(nx+8) doubles (boundary-fill parity checks). */
+int qk_set_raw(qk_ctx *ctx, int field, const double *with_ghosts);
+int qk_get_raw(qk_ctx *ctx, int field, double *with_ghosts);
+
+/* Fill the ghost shell (faces, edges, corners) of the field groups in `which` (QK_FILL_*):
+ * every ghost cell <- the interior cell its three indices map to, periodic wrap or
+ * nearest-interior copy ("B.C. fill"). */
+int qk_fill_boundary(qk_ctx *ctx, int which);
+
+/* eq 21: dt = CFL dx / max_cells(|v| + c_s), |v| the vector magnitude,
+ * further limited to nsub_max CFL dx / c_hat when c_hat > 0.  Synchronises.
+ * Returns NaN if a cell has rho <= 0 or P <= 0 (then qk_last_info().status = QK_ESTATE). */
+double qk_cfl_dt(qk_ctx *ctx);
+
+/* One SSP-RK2 method-of-lines hydro step: per stage ghost fill,
+ * primitives, multidimensional flattening, PPM face states, HLLC fluxes, unsplit update. */
+int qk_hydro_step(qk_ctx *ctx, double dt);
+
+/* SSP-RK2 explicit transport of (E_r, F_r) over dt, no exchange. */
+int qk_rad_transport(qk_ctx *ctx, double dt);
+
+/* Per-cell implicit matter-radiation exchange over dt (eq 26-43). */
+int qk_exchange(qk_ctx *ctx, double dt);
+
+/* ONE radiation subcycle: qk_rad_transport(dt) then qk_exchange(dt). */
+int qk_rad_step(qk_ctx *ctx, double dt);
+
+/* Operator-split cycle: hydro step, then N_sub = max(1, ceil(dt c_hat /
+ * (CFL dx))) radiation subcycles of dt/N_sub.  QK_EINVAL if N_sub > nsub_max. */
+int qk_rhd_step(qk_ctx *ctx, double dt);
+
+/* Number of radiation substeps qk_rhd_step(dt) would take. */
+int qk_nsub_for(const qk_ctx *ctx, double dt);
+
+/* Synchronise and report the counters of the last step call. */
+int qk_last_info(qk_ctx *ctx, qk_info *out);
+
+/* Number of kernel launches this context has enqueued so far (bench.py's gpu_launches). */
+long long qk_launch_count(const qk_ctx *ctx);
+
+/* Which hand-written CUDA implementation of the hydro / radiation stages runs:
+ * QK_PATH_FUSED   = one fused kernel per RK stage (primitives, PPM, Riemann fluxes of the three
+ *                   directions, divergence and stage update; fluxes never reach HBM) -- default;
+ * QK_PATH_UNFUSED = one kernel per sub-step with intermediates in HBM (on-device cross-check).
+ * Both are GPU kernels of this library and give identical results. */
+enum { QK_PATH_FUSED = 0, QK_PATH_UNFUSED = 1 };
+int qk_set_path(qk_ctx *ctx, int path);
+
+/* Per-kernel-class device timing for the roofline report.  While
+ * profiling is on, every group of launches of one kernel class is bracketed by CUDA events on
+ * the context's stream.  qk_kernel_times synchronises, adds the elapsed ms and the number of
+ * bracketed groups per class into ms[]/count[] (arrays of qk_kernel_class_count() entries) and
+ * clears the record. */
+int qk_set_profiling(qk_ctx *ctx, int on);
+int qk_kernel_class_count(void);
+const char *qk_kernel_class_name(int cls);
+int qk_kernel_times(qk_ctx *ctx, double *ms, long long *count);
+
+/* fp64 pipe throughput probe (roofline denominator of the ALU-bound stage kernels, DESIGN.md
+ * section 6): kind 0 = dependent DMUL+DADD chains (the -fmad=false mix the library computes in),
+ * kind 1 = DFMA chains.  Writes fp64 instructions x 32 lanes per second.  Synchronises. */
+int qk_fp64_probe(int kind, int iters, void *cuda_stream, double *lane_ops_per_s);
+
+const char *qk_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QK_H */

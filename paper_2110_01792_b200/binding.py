@@ -1,0 +1,255 @@
+"""Thin ctypes binding of libqk.so (include/qk.h): same names, argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels; PyTorch is used here to hold the
+device allocation (qk_bind_storage) and the stream (qk_set_stream).  There is no CPU path: if
+the library is missing or no CUDA device is present, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libqk.so")
+
+NG = 4
+FIELDS = ["rho", "mx", "my", "mz", "E", "Er", "Fx", "Fy", "Fz", "kappaP", "kappaR"]
+QK_OK, QK_EINVAL, QK_ENOMEM, QK_ECUDA, QK_ENEWTON, QK_ESTATE = range(6)
+QK_BC_PERIODIC, QK_BC_OUTFLOW = 0, 1
+QK_FLAG_TAU_CORR, QK_FLAG_STATIC_MATTER, QK_FLAG_NEWTON_LITERAL = 1, 2, 4
+QK_FILL_HYDRO, QK_FILL_RAD, QK_FILL_OPACITY, QK_FILL_ALL = 1, 2, 4, 7
+QK_PATH_FUSED, QK_PATH_UNFUSED = 0, 1
+
+EXPORTS = [
+    "qk_init", "qk_free", "qk_state_bytes", "qk_bind_storage", "qk_set_stream", "qk_set_constants",
+    "qk_set_params", "qk_set_state", "qk_get_state", "qk_set_raw", "qk_get_raw", "qk_fill_boundary",
+    "qk_cfl_dt", "qk_hydro_step", "qk_rad_transport", "qk_exchange", "qk_rad_step", "qk_rhd_step",
+    "qk_nsub_for", "qk_last_info", "qk_launch_count", "qk_set_path", "qk_set_profiling",
+    "qk_kernel_class_count", "qk_kernel_class_name", "qk_kernel_times", "qk_version", "qk_fp64_probe",
+]
+
+
+class qk_info(C.Structure):
+    _fields_ = [("nsub", C.c_int), ("newton_max_iters", C.c_int), ("newton_fail_cells", C.c_longlong),
+                ("newton_total_iters", C.c_longlong), ("bad_state_cells", C.c_longlong),
+                ("fallback_states", C.c_longlong), ("guard_faces", C.c_longlong), ("status", C.c_int)]
+
+
+class QkError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def lib():
+    """Load libqk.so (built in-tree by paper_2110_01792_b200.build).  Raises if it is absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise QkError("libqk.so is not built: run `python -m paper_2110_01792_b200.build` "
+                      "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    i, d, p, u, ll = C.c_int, C.c_double, C.c_void_p, C.c_uint, C.c_longlong
+    sig = {
+        "qk_init": (i, [i, i, i, d, d, d, d, i, C.POINTER(p)]),
+        "qk_free": (i, [p]),
+        "qk_state_bytes": (C.c_size_t, [i, i, i]),
+        "qk_bind_storage": (i, [p, p, C.c_size_t]),
+        "qk_set_stream": (i, [p, p]),
+        "qk_set_constants": (i, [p, d, d]),
+        "qk_set_params": (i, [p, d, d, i, i, u]),
+        "qk_set_state": (i, [p, i, p]),
+        "qk_get_state": (i, [p, i, p]),
+        "qk_set_raw": (i, [p, i, p]),
+        "qk_get_raw": (i, [p, i, p]),
+        "qk_fill_boundary": (i, [p, i]),
+        "qk_cfl_dt": (d, [p]),
+        "qk_hydro_step": (i, [p, d]),
+        "qk_rad_transport": (i, [p, d]),
+        "qk_exchange": (i, [p, d]),
+        "qk_rad_step": (i, [p, d]),
+        "qk_rhd_step": (i, [p, d]),
+        "qk_nsub_for": (i, [p, d]),
+        "qk_last_info": (i, [p, C.POINTER(qk_info)]),
+        "qk_launch_count": (ll, [p]),
+        "qk_set_path": (i, [p, i]),
+        "qk_set_profiling": (i, [p, i]),
+        "qk_kernel_class_count": (i, []),
+        "qk_kernel_class_name": (C.c_char_p, [i]),
+        "qk_kernel_times": (i, [p, C.POINTER(d), C.POINTER(ll)]),
+        "qk_version": (C.c_char_p, []),
+        "qk_fp64_probe": (i, [i, i, p, C.POINTER(d)]),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(L, name)
+        fn.restype = res
+        fn.argtypes = args
+    _lib = L
+    return L
+
+
+def qk_fp64_probe(kind=0, iters=20000):
+    """fp64 instructions x lanes per second of the fp64 pipe (see include/qk.h)."""
+    import torch
+    out = C.c_double()
+    _check(lib().qk_fp64_probe(kind, iters, C.c_void_p(torch.cuda.current_stream().cuda_stream), C.byref(out)),
+           "qk_fp64_probe")
+    return float(out.value)
+
+
+def _check(rc, what):
+    if rc != QK_OK:
+        names = {1: "QK_EINVAL", 2: "QK_ENOMEM", 3: "QK_ECUDA", 4: "QK_ENEWTON", 5: "QK_ESTATE"}
+        raise QkError("%s failed: %s" % (what, names.get(rc, rc)))
+
+
+def _ptr(a):
+    """Address of a numpy array (host) or torch tensor (host or device), C-contiguous float64."""
+    if isinstance(a, np.ndarray):
+        assert a.dtype == np.float64 and a.flags["C_CONTIGUOUS"]
+        return C.c_void_p(a.ctypes.data)
+    assert a.dtype.is_floating_point and a.element_size() == 8 and a.is_contiguous()
+    return C.c_void_p(a.data_ptr())
+
+
+class Context:
+    """One box on the current CUDA device.  Methods are the C entry points, name for name."""
+
+    def __init__(self, nx, ny, nz, dx, gamma, c_hat=0.0, c=0.0, boundary=QK_BC_PERIODIC, device="cuda:0",
+                 torch_storage=True):
+        import torch
+        if not torch.cuda.is_available():
+            raise QkError("no CUDA device: this library has no CPU path")
+        self.L = lib()
+        self.nx, self.ny, self.nz = nx, ny, nz
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        h = C.c_void_p()
+        _check(self.L.qk_init(nx, ny, nz, dx, gamma, c_hat, c, boundary, C.byref(h)), "qk_init")
+        self.h = h
+        self.storage = None
+        if torch_storage:   # PyTorch owns the device memory
+            nbytes = self.L.qk_state_bytes(nx, ny, nz)
+            self.storage = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            base = self.storage.data_ptr()
+            aligned = (base + 255) // 256 * 256
+            _check(self.L.qk_bind_storage(self.h, C.c_void_p(aligned), nbytes), "qk_bind_storage")
+        self.qk_set_stream(torch.cuda.current_stream(self.device).cuda_stream)
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.L.qk_free(self.h)
+            self.h = None
+            self.storage = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    # ---- one method per C entry point -----------------------------------------------------------
+    def qk_set_stream(self, cuda_stream):
+        _check(self.L.qk_set_stream(self.h, C.c_void_p(cuda_stream)), "qk_set_stream")
+
+    def qk_set_constants(self, a_rad, kB_over_mu_mH):
+        _check(self.L.qk_set_constants(self.h, a_rad, kB_over_mu_mH), "qk_set_constants")
+
+    def qk_set_params(self, cfl=0.3, newton_tol=1e-10, newton_maxit=400, nsub_max=10, flags=QK_FLAG_TAU_CORR):
+        _check(self.L.qk_set_params(self.h, cfl, newton_tol, newton_maxit, nsub_max, flags), "qk_set_params")
+
+    def qk_set_path(self, path):
+        _check(self.L.qk_set_path(self.h, path), "qk_set_path")
+
+    def qk_set_state(self, field, a):
+        assert tuple(a.shape) == (self.nz, self.ny, self.nx), tuple(a.shape)
+        _check(self.L.qk_set_state(self.h, field, _ptr(a)), "qk_set_state")
+
+    def qk_get_state(self, field, out=None):
+        if out is None:
+            out = np.empty((self.nz, self.ny, self.nx), dtype=np.float64)
+        assert tuple(out.shape) == (self.nz, self.ny, self.nx)
+        _check(self.L.qk_get_state(self.h, field, _ptr(out)), "qk_get_state")
+        return out
+
+    def qk_set_raw(self, field, a):
+        assert tuple(a.shape) == (self.nz + 2 * NG, self.ny + 2 * NG, self.nx + 2 * NG)
+        _check(self.L.qk_set_raw(self.h, field, _ptr(a)), "qk_set_raw")
+
+    def qk_get_raw(self, field, out=None):
+        if out is None:
+            out = np.empty((self.nz + 2 * NG, self.ny + 2 * NG, self.nx + 2 * NG), dtype=np.float64)
+        _check(self.L.qk_get_raw(self.h, field, _ptr(out)), "qk_get_raw")
+        return out
+
+    def qk_fill_boundary(self, which=QK_FILL_ALL):
+        _check(self.L.qk_fill_boundary(self.h, which), "qk_fill_boundary")
+
+    def qk_cfl_dt(self):
+        return float(self.L.qk_cfl_dt(self.h))
+
+    def qk_hydro_step(self, dt):
+        _check(self.L.qk_hydro_step(self.h, dt), "qk_hydro_step")
+
+    def qk_rad_transport(self, dt):
+        _check(self.L.qk_rad_transport(self.h, dt), "qk_rad_transport")
+
+    def qk_exchange(self, dt):
+        _check(self.L.qk_exchange(self.h, dt), "qk_exchange")
+
+    def qk_rad_step(self, dt):
+        _check(self.L.qk_rad_step(self.h, dt), "qk_rad_step")
+
+    def qk_rhd_step(self, dt):
+        _check(self.L.qk_rhd_step(self.h, dt), "qk_rhd_step")
+
+    def qk_nsub_for(self, dt):
+        return int(self.L.qk_nsub_for(self.h, dt))
+
+    def qk_last_info(self):
+        info = qk_info()
+        _check(self.L.qk_last_info(self.h, C.byref(info)), "qk_last_info")
+        return {name: int(getattr(info, name)) for name, _ in qk_info._fields_}
+
+    def qk_launch_count(self):
+        return int(self.L.qk_launch_count(self.h))
+
+    def qk_set_profiling(self, on):
+        _check(self.L.qk_set_profiling(self.h, int(on)), "qk_set_profiling")
+
+    def qk_kernel_times(self):
+        n = self.L.qk_kernel_class_count()
+        ms = (C.c_double * n)()
+        cnt = (C.c_longlong * n)()
+        _check(self.L.qk_kernel_times(self.h, ms, cnt), "qk_kernel_times")
+        return {self.L.qk_kernel_class_name(k).decode(): (float(ms[k]), int(cnt[k])) for k in range(n) if cnt[k]}
+
+    # ---- marshalling helpers (no arithmetic) -------------------------------------------------------
+    def set_all(self, fields: dict):
+        for name, a in fields.items():
+            self.qk_set_state(FIELDS.index(name), np.ascontiguousarray(a, dtype=np.float64))
+
+    def get_all(self, names=None):
+        return {n: self.qk_get_state(FIELDS.index(n)) for n in (names or FIELDS)}
+
+
+def from_params(params: dict, fields: dict | None = None, **kw) -> Context:
+    """Context from an inputs.py (params, fields) pair."""
+    ctx = Context(params["nx"], params["ny"], params["nz"], params["dx"], params["gamma"],
+                  params.get("c_hat", 0.0), params.get("c", 0.0), params.get("bc", QK_BC_PERIODIC), **kw)
+    if "a_rad" in params:
+        ctx.qk_set_constants(params["a_rad"], params["kB_mu"])
+    ctx.qk_set_params(cfl=params.get("cfl", 0.3), flags=params.get("flags", QK_FLAG_TAU_CORR))
+    if fields is not None:
+        ctx.set_all(fields)
+    return ctx

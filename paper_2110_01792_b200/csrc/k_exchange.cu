@@ -1,0 +1,64 @@
+// k_exchange.cu -- per-cell implicit matter-radiation exchange, eq 26-43.
+//
+// One thread per interior cell, x fastest so that every field access of a warp is one
+// coalesced 256-byte row segment.  No spatial coupling: the kernel is a pointwise map that
+// reads 11 doubles and writes 8 (152 B/cell) around a Newton loop of a few iterations
+// (HBM-bound).  Counters are reduced per warp before the atomics.
+#include "qk_internal.h"
+#include "qk_math.cuh"
+
+namespace qk {
+
+__global__ void __launch_bounds__(128) exchange_kernel(Geom g, ExchangeConsts kc, double dt, const double *__restrict__ rho,
+                                                       double *__restrict__ mx, double *__restrict__ my,
+                                                       double *__restrict__ mz, double *__restrict__ E,
+                                                       double *__restrict__ Er, double *__restrict__ Fx,
+                                                       double *__restrict__ Fy, double *__restrict__ Fz,
+                                                       const double *__restrict__ kP, const double *__restrict__ kR,
+                                                       Counters *ctr)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y, k = blockIdx.z;
+    int iters = 0, fail = 0, bad = 0;
+    if (i < g.nx) {
+        const int cidx = g.at(i, j, k);
+        double m0 = mx[cidx], m1 = my[cidx], m2 = mz[cidx];
+        double e = E[cidx], er = Er[cidx];
+        double f0 = Fx[cidx], f1 = Fy[cidx], f2 = Fz[cidx];
+        const int rc = exchange_cell(kc, dt, rho[cidx], m0, m1, m2, e, er, f0, f1, f2, kP[cidx], kR[cidx], iters);
+        fail = (rc == 4);
+        bad = (rc == 5);
+        if (!kc.static_matter) { mx[cidx] = m0; my[cidx] = m1; mz[cidx] = m2; }
+        E[cidx] = e; Er[cidx] = er;
+        Fx[cidx] = f0; Fy[cidx] = f1; Fz[cidx] = f2;
+    }
+    int tot = iters, mxit = iters;
+    for (int off = 16; off > 0; off >>= 1) {
+        tot += __shfl_xor_sync(0xffffffffu, tot, off);
+        mxit = max(mxit, __shfl_xor_sync(0xffffffffu, mxit, off));
+        fail += __shfl_xor_sync(0xffffffffu, fail, off);
+        bad += __shfl_xor_sync(0xffffffffu, bad, off);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        if (tot) atomicAdd((unsigned long long *)&ctr->newton_total, (unsigned long long)tot);
+        if (mxit > 0) atomicMax(&ctr->newton_max, mxit);
+        if (fail) atomicAdd((unsigned long long *)&ctr->newton_fail, (unsigned long long)fail);
+        if (bad) atomicAdd((unsigned long long *)&ctr->bad_state, (unsigned long long)bad);
+    }
+}
+
+int launch_exchange(const Geom &g, const PhysConsts &pc, double dt, const double *rho, double *mx, double *my,
+                    double *mz, double *E, double *Er, double *Fx, double *Fy, double *Fz, const double *kP,
+                    const double *kR, Counters *ctr, cudaStream_t st)
+{
+    ExchangeConsts kc;
+    kc.c = pc.c; kc.c_hat = pc.c_hat; kc.a_rad = pc.a_rad; kc.kB_mu = pc.kB_mu; kc.gamma = pc.gamma;
+    kc.tol = pc.newton_tol; kc.maxit = pc.newton_maxit;
+    kc.literal_stop = (pc.flags & QK_FLAG_NEWTON_LITERAL) != 0;
+    kc.static_matter = (pc.flags & QK_FLAG_STATIC_MATTER) != 0;
+    dim3 grid((g.nx + 127) / 128, g.ny, g.nz);
+    exchange_kernel<<<grid, 128, 0, st>>>(g, kc, dt, rho, mx, my, mz, E, Er, Fx, Fy, Fz, kP, kR, ctr);
+    return 1;
+}
+
+}  // namespace qk

@@ -1,0 +1,86 @@
+// qk_internal.h -- layout, context and kernel-launcher declarations shared by the .cu files of
+// libqk (not part of the public ABI; see include/qk.h for that).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <vector>
+
+#include "../../include/qk.h"
+
+namespace qk {
+
+constexpr int NG = QK_NG;
+
+// Box geometry.  Cell (i,j,k) with ghost range -NG..n+NG-1 lives at (k+NG)*sz + (j+NG)*sy + (i+NG).
+struct Geom {
+    int nx, ny, nz;      // interior cells
+    int px, py, pz;      // padded extents n + 2 NG
+    int sy, sz;          // strides in doubles (x stride is 1)
+    int ntot;            // px*py*pz  (<= 2^31: 512^3 boxes are 1.4e8)
+    __host__ __device__ int at(int i, int j, int k) const { return (k + NG) * sz + (j + NG) * sy + (i + NG); }
+};
+
+inline Geom make_geom(int nx, int ny, int nz)
+{
+    Geom g;
+    g.nx = nx; g.ny = ny; g.nz = nz;
+    g.px = nx + 2 * NG; g.py = ny + 2 * NG; g.pz = nz + 2 * NG;
+    g.sy = g.px; g.sz = g.px * g.py;
+    g.ntot = g.px * g.py * g.pz;
+    return g;
+}
+
+// Device-side counters of one public step call (zeroed at its start).
+struct Counters {
+    unsigned long long smax_bits;      // CFL: bit pattern of max(|v|+c_s) (non-negative doubles order as integers)
+    long long cfl_bad;                 // CFL: cells with rho<=0 or P<=0
+    long long bad_state;               // step kernels: cells with rho<=0, P<=0, E_g<=0, E_r<=0
+    long long newton_fail;
+    long long newton_total;
+    long long fallback;
+    long long guard;
+    int newton_max;
+    int pad;
+};
+
+// Kernel classes for per-kernel timing (qk_kernel_times) -- one id per __global__ function family.
+enum KClass { K_FILL = 0, K_CFL, K_PRIM, K_FLATTEN, K_HYDRO_FLUX, K_HYDRO_UPDATE, K_HYDRO_STAGE,
+              K_RAD_PRIM, K_RAD_FLUX, K_RAD_UPDATE, K_RAD_STAGE, K_EXCHANGE, K_NCLASS };
+
+struct PhysConsts {
+    double dx, gamma, c_hat, c, a_rad, kB_mu, cfl, newton_tol;
+    int newton_maxit, nsub_max;
+    unsigned flags;
+    int bc;
+};
+
+// Field pointer bundles passed to kernels by value.
+struct Hydro5 { double *rho, *mx, *my, *mz, *E; };
+struct CHydro5 { const double *rho, *mx, *my, *mz, *E; };
+struct Rad4p { double *E, *Fx, *Fy, *Fz; };
+struct CRad4p { const double *E, *Fx, *Fy, *Fz; };
+
+struct FillList { double *f[QK_NFIELDS]; int n; };
+
+// ---- launchers (each enqueues on `st`; returns the number of kernels launched) -----------------
+int launch_fill(const Geom &g, int bc, const FillList &fl, cudaStream_t st);
+int launch_cfl(const Geom &g, double gamma, CHydro5 U, Counters *ctr, cudaStream_t st);
+
+int launch_prim(const Geom &g, double gamma, CHydro5 U, Hydro5 W, Counters *ctr, cudaStream_t st);
+int launch_flatten(const Geom &g, double gamma, CHydro5 W, double *chi, cudaStream_t st);
+int launch_hydro_flux(const Geom &g, double gamma, int dir, CHydro5 W, const double *chi, Hydro5 flux, cudaStream_t st);
+int launch_hydro_update(const Geom &g, double dtdx, int stage, CHydro5 U, CHydro5 U0, CHydro5 fx, CHydro5 fy,
+                        CHydro5 fz, Hydro5 out, cudaStream_t st);
+
+int launch_rad_prim(const Geom &g, double c, CRad4p R, Rad4p S, Counters *ctr, cudaStream_t st);
+int launch_rad_flux(const Geom &g, const PhysConsts &pc, int dir, CRad4p S, const double *rho, const double *kappaR,
+                    Rad4p flux, Counters *ctr, cudaStream_t st);
+int launch_rad_update(const Geom &g, double dtdx, int stage, CRad4p R, CRad4p R0, CRad4p gx, CRad4p gy, CRad4p gz,
+                      Rad4p out, cudaStream_t st);
+
+int launch_exchange(const Geom &g, const PhysConsts &pc, double dt, const double *rho, double *mx, double *my,
+                    double *mz, double *E, double *Er, double *Fx, double *Fy, double *Fz, const double *kP,
+                    const double *kR, Counters *ctr, cudaStream_t st);
+
+}  // namespace qk

@@ -1,0 +1,337 @@
+"""GPU parity: the CUDA path (through the C ABI, via the ctypes binding) against the CPU oracle on
+the same seeded inputs.  Bars (BASELINE.json north_star): boundary fill and index mapping
+bit-exact; every conserved variable within relative 1e-12 after one step and 1e-9 after 100
+steps (norm: parity_util.rel_errors).  Both implementations avoid FMA contraction and use the
+evaluation order DESIGN.md section 3 fixes, so the observed difference is normally exactly 0."""
+import numpy as np
+import pytest
+
+import oracle as O
+from paper_2110_01792_b200 import binding as B
+from paper_2110_01792_b200 import inputs as I
+
+import parity_util as P
+
+pytestmark = pytest.mark.gpu
+
+PATHS = [B.QK_PATH_FUSED, B.QK_PATH_UNFUSED]
+PATH_IDS = ["fused", "unfused"]
+
+
+# ------------------------------------------------------------------------------------------------
+# S0/S1: layout and boundary fill -- bit-exact
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bc", [B.QK_BC_PERIODIC, B.QK_BC_OUTFLOW])
+@pytest.mark.parametrize("shape", [(32, 32, 32), (19, 22, 37), (1, 1, 16), (2, 3, 5), (4, 4, 64), (5, 1, 1)])
+def test_boundary_fill_bit_exact(shape, bc):
+    nz, ny, nx = shape
+    rng = np.random.default_rng(42)
+    g = O.Grid(nx, ny, nz, 0.1, 5.0 / 3.0, c_hat=1.0, c=10.0, bc=bc)
+    with B.Context(nx, ny, nz, 0.1, 5.0 / 3.0, 1.0, 10.0, bc) as ctx:
+        raws = []
+        for f in range(len(B.FIELDS)):
+            raw = rng.standard_normal((nz + 8, ny + 8, nx + 8))   # ghosts start as garbage
+            g.set_raw(f, raw)
+            ctx.qk_set_raw(f, raw)
+            raws.append(raw)
+        g.fill_boundary(O.FILL_ALL)
+        ctx.qk_fill_boundary(B.QK_FILL_ALL)
+        for f in range(len(B.FIELDS)):
+            ref, got = g.get_raw(f), ctx.qk_get_raw(f)
+            assert np.array_equal(ref.view(np.uint64), got.view(np.uint64)), B.FIELDS[f]
+            # interior untouched
+            assert np.array_equal(got[4:-4, 4:-4, 4:-4], raws[f][4:-4, 4:-4, 4:-4])
+    g.close()
+
+
+def test_fill_groups_are_independent():
+    nz, ny, nx = 6, 7, 9
+    rng = np.random.default_rng(3)
+    with B.Context(nx, ny, nz, 0.1, 1.4, 1.0, 10.0, B.QK_BC_PERIODIC) as ctx:
+        raw = rng.standard_normal((nz + 8, ny + 8, nx + 8))
+        for f in range(len(B.FIELDS)):
+            ctx.qk_set_raw(f, raw)
+        ctx.qk_fill_boundary(B.QK_FILL_RAD)
+        for f in range(len(B.FIELDS)):
+            changed = not np.array_equal(ctx.qk_get_raw(f), raw)
+            assert changed == (5 <= f <= 8), B.FIELDS[f]
+
+
+def test_set_get_state_index_mapping():
+    nz, ny, nx = 5, 6, 11
+    a = np.arange(nz * ny * nx, dtype=np.float64).reshape(nz, ny, nx) + 0.25
+    with B.Context(nx, ny, nz, 0.1, 1.4) as ctx:
+        ctx.qk_set_state(2, a)
+        raw = ctx.qk_get_raw(2)
+        assert np.array_equal(raw[4:-4, 4:-4, 4:-4], a)          # ((k+4)(ny+8)+(j+4))(nx+8)+(i+4)
+        assert np.count_nonzero(raw) == a.size                    # ghosts still zero
+        assert np.array_equal(ctx.qk_get_state(2), a)
+        assert np.count_nonzero(ctx.qk_get_raw(3)) == 0
+
+
+def test_set_get_state_device_pointers():
+    import torch
+    nz, ny, nx = 4, 5, 6
+    a = torch.arange(nz * ny * nx, dtype=torch.float64, device="cuda").reshape(nz, ny, nx) * 0.5
+    with B.Context(nx, ny, nz, 0.1, 1.4) as ctx:
+        ctx.qk_set_state(0, a)
+        out = torch.empty_like(a)
+        ctx.qk_get_state(0, out)
+        assert torch.equal(out, a)
+        assert np.array_equal(ctx.qk_get_state(0), a.cpu().numpy())
+
+
+# ------------------------------------------------------------------------------------------------
+# S2: CFL reduction
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("gen", [lambda: I.config1(), lambda: I.ragged_hydro(), lambda: I.ragged_rhd(),
+                                 lambda: I.config2(n=64)], ids=["config1", "ragged", "ragged_rhd", "turb64"])
+def test_cfl_dt_exact(gen):
+    params, fields = gen()
+    g = P.make_oracle(params, fields)
+    with P.make_gpu(params, fields) as ctx:
+        assert ctx.qk_cfl_dt() == g.cfl_dt()
+    g.close()
+
+
+def test_cfl_dt_bad_state_is_nan():
+    params, fields = I.config1(n=8)
+    fields["rho"][3, 4, 5] = -1.0
+    with P.make_gpu(params, fields) as ctx:
+        assert np.isnan(ctx.qk_cfl_dt())
+
+
+# ------------------------------------------------------------------------------------------------
+# S3-S7: hydro step
+# ------------------------------------------------------------------------------------------------
+def _run_hydro_pair(params, fields, nsteps, path, check_at=()):
+    g = P.make_oracle(params, fields)
+    results = {}
+    with P.make_gpu(params, fields, path=path) as ctx:
+        for s in range(1, nsteps + 1):
+            dt_o, dt_g = g.cfl_dt(), ctx.qk_cfl_dt()
+            assert dt_o == dt_g, (s, dt_o, dt_g)
+            assert g.hydro_step(dt_o) == 0
+            ctx.qk_hydro_step(dt_g)
+            if s in check_at or s == nsteps:
+                results[s] = (g.get_all(I.FIELDS[:5]), ctx.get_all(I.FIELDS[:5]))
+        info = ctx.qk_last_info()
+        assert info["status"] == 0 and info["bad_state_cells"] == 0
+    g.close()
+    return results
+
+
+@pytest.mark.parametrize("path", PATHS, ids=PATH_IDS)
+def test_hydro_config1_one_and_ten_steps(path):
+    """BASELINE.json configs[0]: 32^3 advected wave + noise, 10 SSP-RK2 steps at CFL 0.3."""
+    params, fields = I.config1()
+    res = _run_hydro_pair(params, fields, 10, path, check_at=(1,))
+    P.assert_parity(*res[1], P.TOL_ONE_STEP, P.HYDRO, "config1 step 1")
+    P.assert_parity(*res[10], P.TOL_100_STEPS, P.HYDRO, "config1 step 10")
+
+
+def test_hydro_config1_hundred_steps():
+    params, fields = I.config1()
+    res = _run_hydro_pair(params, fields, 100, B.QK_PATH_FUSED)
+    errs = P.assert_parity(*res[100], P.TOL_100_STEPS, P.HYDRO, "config1 step 100")
+    print("config1, 100 steps, rel errors:", errs)
+
+
+@pytest.mark.parametrize("path", PATHS, ids=PATH_IDS)
+@pytest.mark.parametrize("bc", [B.QK_BC_PERIODIC, B.QK_BC_OUTFLOW], ids=["periodic", "outflow"])
+def test_hydro_ragged_shocks(bc, path):
+    """Non-cubic box that is not a multiple of any tile size, Mach 1.5 (flattening and all HLLC
+    branches active), several tiles plus ragged tails in x, y and z."""
+    params, fields = I.ragged_hydro(bc=bc)
+    res = _run_hydro_pair(params, fields, 5, path, check_at=(1,))
+    P.assert_parity(*res[1], P.TOL_ONE_STEP, P.HYDRO, "ragged step 1")
+    P.assert_parity(*res[5], P.TOL_100_STEPS, P.HYDRO, "ragged step 5")
+
+
+@pytest.mark.parametrize("shape", [(1, 1, 40), (4, 4, 33), (3, 70, 5), (66, 2, 3), (8, 8, 8)])
+def test_hydro_thin_and_tiny_boxes(shape):
+    """Degenerate extents (1-3 cells across, where periodic ghosts wrap several times)."""
+    params, fields = I.ragged_hydro(shape=shape, seed=5)
+    res = _run_hydro_pair(params, fields, 3, B.QK_PATH_FUSED, check_at=(1,))
+    P.assert_parity(*res[1], P.TOL_ONE_STEP, P.HYDRO, "thin %s" % (shape,))
+    P.assert_parity(*res[3], P.TOL_100_STEPS, P.HYDRO, "thin %s" % (shape,))
+
+
+def test_hydro_sedov_small_bitwise():
+    """The paper's hydro benchmark problem at 40^3: strong shock from rest."""
+    params, fields = I.sedov(n=40)
+    res = _run_hydro_pair(params, fields, 8, B.QK_PATH_FUSED)
+    P.assert_parity(*res[8], P.TOL_100_STEPS, P.HYDRO, "sedov")
+    print("sedov mismatching cells:", P.count_mismatch(*res[8], I.FIELDS[:5]))
+
+
+def test_hydro_uniform_state_is_invariant():
+    n = 16
+    shape = (n, n, n)
+    fields = {k: np.zeros(shape) for k in I.FIELDS}
+    fields["rho"][:] = 1.3
+    fields["E"][:] = 2.1
+    params = dict(nx=n, ny=n, nz=n, dx=1.0 / n, gamma=5.0 / 3.0, bc=0)
+    with P.make_gpu(params, fields) as ctx:
+        for _ in range(3):
+            ctx.qk_hydro_step(ctx.qk_cfl_dt())
+        out = ctx.get_all(I.FIELDS[:5])
+    for k in I.FIELDS[:5]:
+        assert np.array_equal(out[k], fields[k]), k
+
+
+# ------------------------------------------------------------------------------------------------
+# S8-S10: radiation transport;  S11-S12: exchange;  S13: drivers
+# ------------------------------------------------------------------------------------------------
+RADF = I.FIELDS[:9]
+
+
+@pytest.mark.parametrize("path", PATHS, ids=PATH_IDS)
+def test_rad_transport_config3_small(path):
+    """BASELINE.json configs[2] generator at 24x20x28: outflow, iid streaming/diffusive mix; the
+    first-order fallback and the tau-correction guard both fire.  Counters are integers: exact."""
+    params, fields = I.config3(shape=(24, 20, 28))
+    g = P.make_oracle(params, fields)
+    dt = 0.3 * params["dx"] / params["c_hat"]
+    with P.make_gpu(params, fields, path=path) as ctx:
+        for s in range(1, 6):
+            assert g.rad_transport(dt) == 0
+            ctx.qk_rad_transport(dt)
+            io, ig = g.info(), ctx.qk_last_info()
+            assert ig["fallback_states"] == io["fallback_states"], s
+            assert ig["guard_faces"] == io["guard_faces"], s
+            if s == 1:
+                assert io["fallback_states"] > 0 and io["guard_faces"] > 0
+                P.assert_parity(g.get_all(RADF), ctx.get_all(RADF), P.TOL_ONE_STEP, P.RAD, "rad step 1")
+        P.assert_parity(g.get_all(RADF), ctx.get_all(RADF), P.TOL_100_STEPS, P.RAD, "rad step 5")
+    g.close()
+
+
+@pytest.mark.parametrize("flags", [1, 3, 5], ids=["default", "static_matter", "literal_stop"])
+def test_exchange_parity_and_counters(flags):
+    params, fields = I.ragged_rhd()
+    params["flags"] = flags
+    g = P.make_oracle(params, fields)
+    with P.make_gpu(params, fields) as ctx:
+        dt = 0.5 * g.cfl_dt()
+        for s in range(3):
+            assert g.exchange(dt) == 0
+            ctx.qk_exchange(dt)
+            io, ig = g.info(), ctx.qk_last_info()
+            for k in ("newton_fail_cells", "newton_max_iters", "newton_total_iters"):
+                assert ig[k] == io[k], (k, s)
+        P.assert_parity(g.get_all(RADF), ctx.get_all(RADF), P.TOL_ONE_STEP, None, "exchange")
+    g.close()
+
+
+def test_exchange_newton_cap_is_reported():
+    params, fields = I.ragged_rhd()
+    g = P.make_oracle(params, fields)
+    g.set_params(newton_maxit=1, flags=params["flags"])
+    with P.make_gpu(params, fields) as ctx:
+        ctx.qk_set_params(newton_maxit=1, flags=params["flags"])
+        dt = g.cfl_dt()
+        g.exchange(dt)
+        ctx.qk_exchange(dt)
+        io, ig = g.info(), ctx.qk_last_info()
+        assert ig["newton_fail_cells"] == io["newton_fail_cells"] > 0
+        assert ig["status"] == B.QK_ENEWTON
+    g.close()
+
+
+@pytest.mark.parametrize("path", PATHS, ids=PATH_IDS)
+@pytest.mark.parametrize("bc", [B.QK_BC_PERIODIC, B.QK_BC_OUTFLOW], ids=["periodic", "outflow"])
+def test_rhd_step_ragged(bc, path):
+    """Full operator-split cycle (hydro, N_sub x (transport, exchange)) on a ragged box."""
+    params, fields = I.ragged_rhd(bc=bc)
+    g = P.make_oracle(params, fields)
+    with P.make_gpu(params, fields, path=path) as ctx:
+        for s in range(1, 5):
+            dt_o, dt_g = g.cfl_dt(), ctx.qk_cfl_dt()
+            assert dt_o == dt_g
+            assert g.rhd_step(dt_o) == 0
+            ctx.qk_rhd_step(dt_g)
+            io, ig = g.info(), ctx.qk_last_info()
+            assert ig["nsub"] == io["nsub"] == g.nsub_for(dt_o) == ctx.qk_nsub_for(dt_g)
+            for k in ("newton_fail_cells", "newton_max_iters", "newton_total_iters", "fallback_states",
+                      "guard_faces"):
+                assert ig[k] == io[k], (k, s)
+            if s == 1:
+                P.assert_parity(g.get_all(RADF), ctx.get_all(RADF), P.TOL_ONE_STEP, None, "rhd step 1")
+        P.assert_parity(g.get_all(RADF), ctx.get_all(RADF), P.TOL_100_STEPS, None, "rhd step 4")
+    g.close()
+
+
+def test_rhd_subcycling_nsub_gt_1():
+    """c_hat large enough that dt_hydro needs several radiation substeps."""
+    params, fields = I.ragged_rhd()
+    params["c_hat"] = params["c_hat"] * 4.0
+    g = P.make_oracle(params, fields)
+    with P.make_gpu(params, fields) as ctx:
+        dt = g.cfl_dt()
+        assert ctx.qk_cfl_dt() == dt
+        assert g.nsub_for(dt) > 1
+        assert g.rhd_step(dt) == 0
+        ctx.qk_rhd_step(dt)
+        assert ctx.qk_last_info()["nsub"] == g.info()["nsub"] > 1
+        P.assert_parity(g.get_all(RADF), ctx.get_all(RADF), P.TOL_ONE_STEP, None, "rhd nsub>1")
+    g.close()
+
+
+def test_rad_step_config3_fifty_substeps():
+    """BASELINE.json configs[2] recipe (50 substeps, static matter, outflow) at 20^3."""
+    params, fields = I.config3(shape=(20, 20, 20))
+    g = P.make_oracle(params, fields)
+    dt = 0.3 * params["dx"] / params["c_hat"]
+    with P.make_gpu(params, fields) as ctx:
+        for s in range(50):
+            assert g.rad_step(dt) == 0
+            ctx.qk_rad_step(dt)
+        P.assert_parity(g.get_all(RADF), ctx.get_all(RADF), P.TOL_100_STEPS, None, "config3 50 substeps")
+        assert ctx.qk_last_info()["status"] == 0
+    g.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# Full-size configs in bench.py's launch configuration, checked on sampled sub-boxes
+# ------------------------------------------------------------------------------------------------
+def _sampled_full_size(params, fields, stepper_gpu, stepper_orc, names, tol, halo, core=6, nsamples=4, seed=9):
+    """One step of the full-size box on the GPU; for a few sample locations the oracle advances a
+    (core+2*halo)^3 sub-box cut (periodically) from the same input and the core cells, whose
+    domain of dependence lies inside the sub-box, must agree."""
+    n = params["nx"]
+    rng = np.random.default_rng(seed)
+    los = [(0, 0, 0), (n - halo - 3, n - halo - 2, n - halo - 1)]        # straddle the periodic wrap
+    los += [tuple(int(v) for v in rng.integers(0, n, 3)) for _ in range(nsamples - 2)]
+    size = (core + 2 * halo,) * 3
+    with P.make_gpu(params, fields) as ctx:
+        dt = ctx.qk_cfl_dt()
+        stepper_gpu(ctx, dt)
+        got = ctx.get_all(names)
+        assert ctx.qk_last_info()["status"] == 0
+    for lo in los:
+        sub_p = dict(params, nx=size[2], ny=size[1], nz=size[0], bc=B.QK_BC_OUTFLOW)
+        g = P.make_oracle(sub_p, P.sub_box(fields, lo, size))
+        assert stepper_orc(g, dt) == 0
+        ref = g.get_all(names)
+        g.close()
+        gsub = P.sub_box(got, lo, size)
+        sl = (slice(halo, halo + core),) * 3
+        P.assert_parity({k: ref[k][sl] for k in names}, {k: gsub[k][sl] for k in names}, tol,
+                        [k for k, v in P.GROUPS.items() if all(n_ in names for n_ in v)],
+                        "full-size sample at %s" % (lo,))
+
+
+def test_hydro_config2_full_size_sampled():
+    """BASELINE.json configs[1] (256^3 Mach-2 turbulence): one step at full size, sampled."""
+    params, fields = I.config2()
+    _sampled_full_size(params, fields, lambda c, dt: c.qk_hydro_step(dt), lambda g, dt: g.hydro_step(dt),
+                       I.FIELDS[:5], P.TOL_ONE_STEP, halo=8)
+
+
+def test_rhd_config4_full_size_sampled():
+    """BASELINE.json configs[3] (256^3 coupled RHD): one full cycle at full size, sampled.
+    Domain of dependence: 2 hydro stages x 4 + N_sub=1 x 2 radiation stages x 3 = 14 cells."""
+    params, fields = I.config4()
+    _sampled_full_size(params, fields, lambda c, dt: c.qk_rhd_step(dt), lambda g, dt: g.rhd_step(dt),
+                       I.FIELDS[:9], P.TOL_ONE_STEP, halo=14, core=4, nsamples=3)
