@@ -177,15 +177,28 @@ void hydro_stage_unfused(qk_ctx *c, double dtdx, int stage, double *const *U, do
     }
 }
 
+void hydro_stage_fused(qk_ctx *c, double dtdx, int stage, double *const *U, double *const *U0, double *const *out)
+{
+    const Geom &g = c->g;
+    { Scope s(c, K_FLATTEN); s.done(launch_flatten_march(g, c->pc.gamma, ch5(U), c->chi, c->stream)); }
+    {
+        Scope s(c, K_HYDRO_STAGE);
+        s.done(launch_hydro_stage(g, c->pc.gamma, dtdx, stage, ch5(U), ch5(U0), c->chi, h5(out), c->ctr, c->stream));
+    }
+}
+
 int do_hydro_step(qk_ctx *c, double dt)
 {
     const double dtdx = dt / c->pc.dx;
     double *const *Un = &c->state[QK_RHO];
     double *const *U1 = &c->stage[0];
+    const bool fused = c->path == QK_PATH_FUSED;
     fill_fields(c, Un, 5);
-    hydro_stage_unfused(c, dtdx, 0, Un, Un, U1);
+    if (fused) hydro_stage_fused(c, dtdx, 0, Un, Un, U1);
+    else       hydro_stage_unfused(c, dtdx, 0, Un, Un, U1);
     fill_fields(c, U1, 5);
-    hydro_stage_unfused(c, dtdx, 1, U1, Un, Un);
+    if (fused) hydro_stage_fused(c, dtdx, 1, U1, Un, Un);
+    else       hydro_stage_unfused(c, dtdx, 1, U1, Un, Un);
     return check_launch();
 }
 
@@ -268,7 +281,7 @@ int qk_init(int nx, int ny, int nz, double dx, double gamma, double c_hat, doubl
     x->pc.a_rad = 1.0; x->pc.kB_mu = 1.0; x->pc.cfl = 0.3; x->pc.newton_tol = 1e-10;
     x->pc.newton_maxit = 400; x->pc.nsub_max = 10; x->pc.flags = QK_FLAG_TAU_CORR; x->pc.bc = boundary;
     x->stream = nullptr; x->device = dev; x->base = nullptr; x->bytes = 0; x->owns = false; x->ready = false;
-    x->path = QK_PATH_UNFUSED; x->launches = 0; x->last_nsub = 0; x->profiling = false;
+    x->path = QK_PATH_FUSED; x->launches = 0; x->last_nsub = 0; x->profiling = false;
     *out = x;
     return QK_OK;
 }

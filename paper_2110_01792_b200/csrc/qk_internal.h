@@ -73,6 +73,11 @@ int launch_hydro_flux(const Geom &g, double gamma, int dir, CHydro5 W, const dou
 int launch_hydro_update(const Geom &g, double dtdx, int stage, CHydro5 U, CHydro5 U0, CHydro5 fx, CHydro5 fy,
                         CHydro5 fz, Hydro5 out, cudaStream_t st);
 
+// fused path (k_hydro.cu, k_rad.cu)
+int launch_flatten_march(const Geom &g, double gamma, CHydro5 U, double *chi, cudaStream_t st);
+int launch_hydro_stage(const Geom &g, double gamma, double dtdx, int stage, CHydro5 U, CHydro5 U0, const double *chi,
+                       Hydro5 out, Counters *ctr, cudaStream_t st);
+
 int launch_rad_prim(const Geom &g, double c, CRad4p R, Rad4p S, Counters *ctr, cudaStream_t st);
 int launch_rad_flux(const Geom &g, const PhysConsts &pc, int dir, CRad4p S, const double *rho, const double *kappaR,
                     Rad4p flux, Counters *ctr, cudaStream_t st);
