@@ -223,6 +223,13 @@ void rad_stage_unfused(qk_ctx *c, double dtdx, int stage, double *const *R, doub
     }
 }
 
+void rad_stage_fused(qk_ctx *c, double dtdx, int stage, double *const *R, double *const *R0, double *const *out)
+{
+    Scope s(c, K_RAD_STAGE);
+    s.done(launch_rad_stage(c->g, c->pc, dtdx, stage, cr4(R), cr4(R0), c->state[QK_RHO], c->state[QK_KAPPA_R], r4(out),
+                            c->ctr, c->stream));
+}
+
 int do_rad_transport(qk_ctx *c, double dt)
 {
     const double dtdx = dt / c->pc.dx;
@@ -230,10 +237,13 @@ int do_rad_transport(qk_ctx *c, double dt)
     double *const *R1 = &c->stage[0];
     // rho and kappa_R ghosts feed tau_face at the domain faces
     double *first[6] = {Rn[0], Rn[1], Rn[2], Rn[3], c->state[QK_RHO], c->state[QK_KAPPA_R]};
+    const bool fused = c->path == QK_PATH_FUSED;
     fill_fields(c, first, 6);
-    rad_stage_unfused(c, dtdx, 0, Rn, Rn, R1);
+    if (fused) rad_stage_fused(c, dtdx, 0, Rn, Rn, R1);
+    else       rad_stage_unfused(c, dtdx, 0, Rn, Rn, R1);
     fill_fields(c, R1, 4);
-    rad_stage_unfused(c, dtdx, 1, R1, Rn, Rn);
+    if (fused) rad_stage_fused(c, dtdx, 1, R1, Rn, Rn);
+    else       rad_stage_unfused(c, dtdx, 1, R1, Rn, Rn);
     return check_launch();
 }
 

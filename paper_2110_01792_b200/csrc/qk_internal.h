@@ -78,6 +78,9 @@ int launch_flatten_march(const Geom &g, double gamma, CHydro5 U, double *chi, cu
 int launch_hydro_stage(const Geom &g, double gamma, double dtdx, int stage, CHydro5 U, CHydro5 U0, const double *chi,
                        Hydro5 out, Counters *ctr, cudaStream_t st);
 
+int launch_rad_stage(const Geom &g, const PhysConsts &pc, double dtdx, int stage, CRad4p R, CRad4p R0, const double *rho,
+                     const double *kappaR, Rad4p out, Counters *ctr, cudaStream_t st);
+
 int launch_rad_prim(const Geom &g, double c, CRad4p R, Rad4p S, Counters *ctr, cudaStream_t st);
 int launch_rad_flux(const Geom &g, const PhysConsts &pc, int dir, CRad4p S, const double *rho, const double *kappaR,
                     Rad4p flux, Counters *ctr, cudaStream_t st);
