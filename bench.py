@@ -221,7 +221,7 @@ def time_steps_e2e(torch, ctx, kind, nsteps, host_in, host_out, barrier):
     return e0.elapsed_time(e1)
 
 
-def run_workload(torch, B, I, kind, n, steps, warmup, rank, world, barrier, allmax, sampler=None):
+def run_workload(torch, B, I, kind, n, steps, warmup, rank, world, barrier, allmax, sampler=None, path=None):
     t0 = time.time()
     params, fields = (I.config2(n=n, seed=1002 + rank) if kind == "hydro" else I.config4(n=n, seed=1004 + rank))
     log("[rank %d] %s %d^3 inputs generated in %.1f s" % (rank, kind, n, time.time() - t0))
@@ -229,6 +229,8 @@ def run_workload(torch, B, I, kind, n, steps, warmup, rank, world, barrier, allm
     cells = n ** 3
     out = {}
     with B.from_params(params, fields) as ctx:
+        if path is not None:
+            ctx.qk_set_path(path)
         for _ in range(warmup):
             dt = ctx.qk_cfl_dt()
             ctx.qk_hydro_step(dt) if kind == "hydro" else ctx.qk_rhd_step(dt)
@@ -315,11 +317,12 @@ def run_ours(args):
     hbm_note = "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
 
     sampler = ClockSampler(local) if rank == 0 else None
-    hyd = run_workload(torch, B, I, "hydro", n, args.steps, args.warmup, rank, world, barrier, allmax, sampler)
+    path = {"fused": B.QK_PATH_FUSED, "unfused": B.QK_PATH_UNFUSED, "sweep": B.QK_PATH_SWEEP}[args.path]
+    hyd = run_workload(torch, B, I, "hydro", n, args.steps, args.warmup, rank, world, barrier, allmax, sampler, path)
     rhd = None
     if not args.no_rhd:
         rhd_steps = max(1, min(args.steps, args.rhd_steps))
-        rhd = run_workload(torch, B, I, "rhd", n, rhd_steps, min(args.warmup, 3), rank, world, barrier, allmax)
+        rhd = run_workload(torch, B, I, "rhd", n, rhd_steps, min(args.warmup, 3), rank, world, barrier, allmax, None, path)
         rhd["steps"] = rhd_steps
 
     if rank != 0:
@@ -389,6 +392,7 @@ def main():
     ap.add_argument("--size", type=int, default=256, help="box edge (BASELINE metric: 256)")
     ap.add_argument("--rhd-steps", type=int, default=10)
     ap.add_argument("--ref-size", type=int, default=128, help="edge of the oracle's bounded sample")
+    ap.add_argument("--path", default="fused", choices=["fused", "unfused", "sweep"], help="stage kernel family")
     ap.add_argument("--no-rhd", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -140,11 +140,13 @@ int qk_last_info(qk_ctx *ctx, qk_info *out);
 long long qk_launch_count(const qk_ctx *ctx);
 
 /* Which hand-written CUDA implementation of the hydro / radiation stages runs:
- * QK_PATH_FUSED   = one fused kernel per RK stage (primitives, PPM, Riemann fluxes of the three
- *                   directions, divergence and stage update; fluxes never reach HBM) -- default;
- * QK_PATH_UNFUSED = one kernel per sub-step with intermediates in HBM (on-device cross-check).
- * Both are GPU kernels of this library and give identical results. */
-enum { QK_PATH_FUSED = 0, QK_PATH_UNFUSED = 1 };
+ * QK_PATH_FUSED   = one tiled kernel per RK stage (primitives, PPM, Riemann fluxes of the three
+ *                   directions, divergence and stage update; fluxes never reach HBM);
+ * QK_PATH_UNFUSED = one kernel per sub-step with intermediates in HBM (on-device cross-check);
+ * QK_PATH_SWEEP   = direction-split barrier-free sweeps (x by warp shuffle, y and z by marching
+ *                   columns), flux differences accumulated in one scratch field per variable.
+ * All are GPU kernels of this library and give bit-identical results (same evaluation order). */
+enum { QK_PATH_FUSED = 0, QK_PATH_UNFUSED = 1, QK_PATH_SWEEP = 2 };
 int qk_set_path(qk_ctx *ctx, int path);
 
 /* Per-kernel-class device timing for the roofline report.  While

@@ -21,8 +21,8 @@ LIB = os.path.join(HERE, "libqk.so")
 OBJ = os.path.join(HERE, "build")
 
 SOURCES = ["qk_api.cu", "k_boundary.cu", "k_cfl.cu", "k_exchange.cu", "k_hydro_ref.cu", "k_rad_ref.cu",
-           "k_hydro.cu", "k_rad.cu", "k_peak.cu"]
-HEADERS = ["qk_internal.h", "qk_math.cuh", "k_stage_common.cuh"]
+           "k_hydro.cu", "k_rad.cu", "k_sweep.cu", "k_peak.cu"]
+HEADERS = ["qk_internal.h", "qk_math.cuh", "k_stage_common.cuh", "k_sweep.cuh"]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-fmad=false",
               "-std=c++17", "-Xcompiler", "-fPIC"]

@@ -162,30 +162,6 @@ struct HydroSmem {
     double loYe[5][TX];                             // low-y face state of cell TY
 };
 
-// flattened PPM face states of all five primitives of one cell; q(v, m) = value of variable v at
-// stencil offset m-2
-template <typename Q>
-__device__ __forceinline__ void ppm_cell(Q q, double chi, double lo[5], double hi[5])
-{
-#pragma unroll
-    for (int v = 0; v < 5; ++v) {
-        const double c = q(v, 2);
-        double l, h;
-        ppm_face_states(q(v, 0), q(v, 1), c, q(v, 3), q(v, 4), l, h);
-        lo[v] = c + chi * (l - c);          // flatten toward the cell average
-        hi[v] = c + chi * (h - c);
-    }
-}
-
-// HLLC flux through a face with normal DIR; L, R = (rho, vx, vy, vz, P); F in conserved order
-template <int DIR>
-__device__ __forceinline__ void face_flux(double gamma, const double L[5], const double R[5], double F[5])
-{
-    constexpr int n = 1 + DIR, t1 = 1 + (DIR + 1) % 3, t2 = 1 + (DIR + 2) % 3;
-    const Flux5 f = hllc_flux(gamma, L[0], L[n], L[t1], L[t2], L[4], R[0], R[n], R[t1], R[t2], R[4]);
-    F[0] = f.m; F[n] = f.pn; F[t1] = f.pt1; F[t2] = f.pt2; F[4] = f.e;
-}
-
 __global__ void __launch_bounds__(NT, 2) hydro_stage_kernel(Geom g, double gamma, double dtdx, int stage, CHydro5 U,
                                                             CHydro5 U0, const double *__restrict__ chi, Hydro5 out,
                                                             int lz, Counters *ctr)

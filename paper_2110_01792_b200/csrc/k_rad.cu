@@ -48,44 +48,6 @@ struct RadSmem {
     double loYe[4][TX];                             // low-y face state of cell TY
 };
 
-// PPM face states of (E, fx, fy, fz) of one cell, q(v, m) = variable v at stencil offset m-2; a face
-// state with |f|^2 > 1 or E <= 0 reverts to the cell average.  Returns the number of
-// reverted states.
-template <typename Q>
-__device__ __forceinline__ int rad_ppm_cell(Q q, double lo[4], double hi[4])
-{
-    double ctr[4];
-#pragma unroll
-    for (int v = 0; v < 4; ++v) {
-        ctr[v] = q(v, 2);
-        ppm_face_states(q(v, 0), q(v, 1), ctr[v], q(v, 3), q(v, 4), lo[v], hi[v]);
-    }
-    int nfall = 0;
-    double f2 = (lo[1] * lo[1] + lo[2] * lo[2]) + lo[3] * lo[3];
-    if (f2 > 1.0 || !(lo[0] > 0.0)) {
-#pragma unroll
-        for (int v = 0; v < 4; ++v) lo[v] = ctr[v];
-        ++nfall;
-    }
-    f2 = (hi[1] * hi[1] + hi[2] * hi[2]) + hi[3] * hi[3];
-    if (f2 > 1.0 || !(hi[0] > 0.0)) {
-#pragma unroll
-        for (int v = 0; v < 4; ++v) hi[v] = ctr[v];
-        ++nfall;
-    }
-    return nfall;
-}
-
-template <int DIR>
-__device__ __forceinline__ int rad_face_flux(double c, double c_hat, bool tau_corr, double tau, const double L[4],
-                                             const double R[4], double G[4])
-{
-    int guard;
-    const Rad4 g = rad_hll_flux(c, c_hat, L[0], L[1], L[2], L[3], R[0], R[1], R[2], R[3], DIR, tau, tau_corr, guard);
-    G[0] = g.e; G[1] = g.x; G[2] = g.y; G[3] = g.z;
-    return guard;
-}
-
 __global__ void __launch_bounds__(NT, 2) rad_stage_kernel(Geom g, double c, double c_hat, double dx, int tau_corr_i,
                                                           double dtdx, int stage, CRad4p R, CRad4p R0,
                                                           const double *__restrict__ rho, const double *__restrict__ kR,

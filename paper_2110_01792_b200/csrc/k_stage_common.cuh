@@ -11,6 +11,7 @@
 #pragma once
 
 #include "qk_internal.h"
+#include "qk_math.cuh"
 
 namespace qk {
 
@@ -65,6 +66,70 @@ __device__ __forceinline__ void edge_cell(int e, int &lx, int &ly, bool &along_x
 __device__ __forceinline__ bool in_array(const Geom &g, int i, int j)
 {
     return i >= -NG && i < g.nx + NG && j >= -NG && j < g.ny + NG;
+}
+
+// ---- per-cell / per-face building blocks shared by the tile kernels and the sweep kernels ------
+
+// flattened PPM face states of all five primitives of one cell; q(v, m) = value of variable v at
+// stencil offset m-2
+template <typename Q>
+__device__ __forceinline__ void ppm_cell(Q q, double chi, double lo[5], double hi[5])
+{
+#pragma unroll
+    for (int v = 0; v < 5; ++v) {
+        const double c = q(v, 2);
+        double l, h;
+        ppm_face_states(q(v, 0), q(v, 1), c, q(v, 3), q(v, 4), l, h);
+        lo[v] = c + chi * (l - c);          // flatten toward the cell average
+        hi[v] = c + chi * (h - c);
+    }
+}
+
+// HLLC flux through a face with normal DIR; L, R = (rho, vx, vy, vz, P); F in conserved order
+template <int DIR>
+__device__ __forceinline__ void face_flux(double gamma, const double L[5], const double R[5], double F[5])
+{
+    constexpr int n = 1 + DIR, t1 = 1 + (DIR + 1) % 3, t2 = 1 + (DIR + 2) % 3;
+    const Flux5 f = hllc_flux(gamma, L[0], L[n], L[t1], L[t2], L[4], R[0], R[n], R[t1], R[t2], R[4]);
+    F[0] = f.m; F[n] = f.pn; F[t1] = f.pt1; F[t2] = f.pt2; F[4] = f.e;
+}
+
+// PPM face states of (E, fx, fy, fz) of one cell, q(v, m) = variable v at stencil offset m-2; a face
+// state with |f|^2 > 1 or E <= 0 reverts to the cell average.  Returns the number of
+// reverted states.
+template <typename Q>
+__device__ __forceinline__ int rad_ppm_cell(Q q, double lo[4], double hi[4])
+{
+    double ctr[4];
+#pragma unroll
+    for (int v = 0; v < 4; ++v) {
+        ctr[v] = q(v, 2);
+        ppm_face_states(q(v, 0), q(v, 1), ctr[v], q(v, 3), q(v, 4), lo[v], hi[v]);
+    }
+    int nfall = 0;
+    double f2 = (lo[1] * lo[1] + lo[2] * lo[2]) + lo[3] * lo[3];
+    if (f2 > 1.0 || !(lo[0] > 0.0)) {
+#pragma unroll
+        for (int v = 0; v < 4; ++v) lo[v] = ctr[v];
+        ++nfall;
+    }
+    f2 = (hi[1] * hi[1] + hi[2] * hi[2]) + hi[3] * hi[3];
+    if (f2 > 1.0 || !(hi[0] > 0.0)) {
+#pragma unroll
+        for (int v = 0; v < 4; ++v) hi[v] = ctr[v];
+        ++nfall;
+    }
+    return nfall;
+}
+
+template <int DIR>
+__device__ __forceinline__ int rad_face_flux(double c, double c_hat, bool tau_corr, double tau, const double L[4],
+                                             const double R[4], double G[4])
+{
+    int guard;
+    const Rad4 g = rad_hll_flux(c, c_hat, L[0], L[1], L[2], L[3], R[0], R[1], R[2], R[3], DIR, tau, tau_corr, guard);
+    G[0] = g.e; G[1] = g.x; G[2] = g.y; G[3] = g.z;
+    return guard;
 }
 
 }  // namespace qk

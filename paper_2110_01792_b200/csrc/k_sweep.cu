@@ -1,0 +1,127 @@
+// k_sweep.cu -- physics policies and launchers of the direction-split sweep path (k_sweep.cuh).
+//
+// Hydro stage:  prim (cons -> rho, v, P, all cells)  ->  chi (flattening, H6)
+//   -> x sweep (D = dFx) -> y sweep (D += dFy) -> z sweep (U' = RK(U, (dFx+dFy)+dFz)).
+// Radiation stage:  rad prim (E_r, f = F_r/(c E_r))  -> x, y, z sweeps the same way.
+#include <stdlib.h>
+
+#include "k_sweep.cuh"
+
+namespace qk {
+
+// ---- hydro ------------------------------------------------------------------------------------------
+struct HydroPh {
+    static constexpr int NV = 5;
+    static constexpr bool COUNTS = false;
+    const double *w[5];        // rho, vx, vy, vz, P (ghost cells included)
+    const double *chi;         // flattening coefficient of the cells -1..n
+    double gamma;
+    __device__ __forceinline__ double ld(int v, int cidx) const { return __ldg(w[v] + cidx); }
+    __device__ __forceinline__ double aux(int cidx) const { return __ldg(chi + cidx); }
+    template <class Q>
+    __device__ __forceinline__ int states(Q q, double x, double lo[5], double hi[5]) const
+    {
+        ppm_cell(q, x, lo, hi);
+        return 0;
+    }
+    template <int DIR>
+    __device__ __forceinline__ int flux(const double L[5], const double R[5], double, double, double F[5]) const
+    {
+        face_flux<DIR>(gamma, L, R, F);
+        return 0;
+    }
+};
+
+// ---- radiation --------------------------------------------------------------------------------------
+struct RadPh {
+    static constexpr int NV = 4;
+    static constexpr bool COUNTS = true;
+    const double *s[4];        // E_r, fx, fy, fz
+    const double *rho, *kR;
+    double c, c_hat, dx;
+    int tau_corr;
+    __device__ __forceinline__ double ld(int v, int cidx) const
+    {
+        if (v < 4) return __ldg(s[v] + cidx);
+        return __ldg(kR + cidx) * __ldg(rho + cidx);      // kappa_R rho of the cell
+    }
+    __device__ __forceinline__ double aux(int) const { return 0.0; }
+    template <class Q>
+    __device__ __forceinline__ int states(Q q, double, double lo[4], double hi[4]) const
+    {
+        return rad_ppm_cell(q, lo, hi);
+    }
+    template <int DIR>
+    __device__ __forceinline__ int flux(const double L[4], const double R[4], double krL, double krR, double G[4]) const
+    {
+        const double tau = (0.5 * (krL + krR)) * dx;
+        return rad_face_flux<DIR>(c, c_hat, tau_corr != 0, tau, L, R, G);
+    }
+};
+
+static int sweep_len(int n_m, long long columns)
+{
+    static int forced = -1;
+    if (forced < 0) {
+        const char *e = getenv("QK_SWEEP_LEN");
+        forced = e ? atoi(e) : 0;
+    }
+    int len = forced > 0 ? forced : 32;
+    // keep at least ~8 waves of warps on 148 SMs x 16 warps
+    while (forced <= 0 && len > 8 && columns / 32 * ((n_m + len - 1) / len) < 148LL * 16 * 8) len /= 2;
+    if (len > n_m) len = n_m;
+    return len < 1 ? 1 : len;
+}
+
+template <class PH>
+static int launch_sweeps(const PH &ph, const Geom &g, double dtdx, int stage, FieldsRW<PH::NV> D, FieldsRO<PH::NV> U,
+                         FieldsRO<PH::NV> U0, FieldsRW<PH::NV> out, Counters *ctr, cudaStream_t st, int which)
+{
+    const RkArgs rk{dtdx, stage};
+    int n = 0;
+    if (which & 1) {
+        dim3 grid((g.nx + SW_XW - 1) / SW_XW, (g.ny + SW_XROWS - 1) / SW_XROWS, g.nz), block(32, SW_XROWS);
+        sweep_x_kernel<PH><<<grid, block, 0, st>>>(ph, g, D, ctr);
+        ++n;
+    }
+    const int bx = (g.nx + SW_NT - 1) / SW_NT;
+    if (which & 2) {
+        const int len = sweep_len(g.ny, (long long)g.nx * g.nz);
+        dim3 grid(bx, g.nz, (g.ny + len - 1) / len);
+        sweep_march_kernel<PH, 1, 1><<<grid, SW_NT, 0, st>>>(ph, g, len, D, rk, U, U0, out, ctr);
+        ++n;
+    }
+    if (which & 4) {
+        const int len = sweep_len(g.nz, (long long)g.nx * g.ny);
+        dim3 grid(bx, g.ny, (g.nz + len - 1) / len);
+        sweep_march_kernel<PH, 2, 2><<<grid, SW_NT, 0, st>>>(ph, g, len, D, rk, U, U0, out, ctr);
+        ++n;
+    }
+    return n;
+}
+
+int launch_hydro_sweeps(const Geom &g, double gamma, double dtdx, int stage, CHydro5 W, const double *chi, Hydro5 D,
+                        CHydro5 U, CHydro5 U0, Hydro5 out, Counters *ctr, cudaStream_t st, int which)
+{
+    HydroPh ph;
+    ph.w[0] = W.rho; ph.w[1] = W.mx; ph.w[2] = W.my; ph.w[3] = W.mz; ph.w[4] = W.E;
+    ph.chi = chi; ph.gamma = gamma;
+    FieldsRW<5> d{{D.rho, D.mx, D.my, D.mz, D.E}}, o{{out.rho, out.mx, out.my, out.mz, out.E}};
+    FieldsRO<5> u{{U.rho, U.mx, U.my, U.mz, U.E}}, u0{{U0.rho, U0.mx, U0.my, U0.mz, U0.E}};
+    return launch_sweeps(ph, g, dtdx, stage, d, u, u0, o, ctr, st, which);
+}
+
+int launch_rad_sweeps(const Geom &g, const PhysConsts &pc, double dtdx, int stage, CRad4p S, const double *rho,
+                      const double *kappaR, Rad4p D, CRad4p R, CRad4p R0, Rad4p out, Counters *ctr, cudaStream_t st,
+                      int which)
+{
+    RadPh ph;
+    ph.s[0] = S.E; ph.s[1] = S.Fx; ph.s[2] = S.Fy; ph.s[3] = S.Fz;
+    ph.rho = rho; ph.kR = kappaR;
+    ph.c = pc.c; ph.c_hat = pc.c_hat; ph.dx = pc.dx; ph.tau_corr = (pc.flags & QK_FLAG_TAU_CORR) ? 1 : 0;
+    FieldsRW<4> d{{D.E, D.Fx, D.Fy, D.Fz}}, o{{out.E, out.Fx, out.Fy, out.Fz}};
+    FieldsRO<4> u{{R.E, R.Fx, R.Fy, R.Fz}}, u0{{R0.E, R0.Fx, R0.Fy, R0.Fz}};
+    return launch_sweeps(ph, g, dtdx, stage, d, u, u0, o, ctr, st, which);
+}
+
+}  // namespace qk

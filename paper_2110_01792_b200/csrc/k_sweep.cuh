@@ -1,0 +1,178 @@
+// k_sweep.cuh -- direction-split, barrier-free sweep kernels shared by the hydro and radiation stages.
+//
+// The stage kernels are bound by the fp64 pipe, not by HBM: at 100 % pipe
+// utilisation a stage could move ~500 B/cell before HBM mattered.  The sweeps therefore trade a few
+// hundred bytes per cell of extra traffic for instruction streams that never wait on another warp:
+//
+//   sweep_x_kernel     : one thread per cell, one warp per x row segment.  Lane l owns cell
+//                        30 b - 1 + l; the high face state of the left neighbour and the flux of the
+//                        right neighbour arrive by warp shuffle, so lanes 1..30 produce a flux
+//                        difference and lanes 0, 31 are halo lanes.  Writes D = dF_x.
+//   sweep_march_kernel : one thread per (x, other) column, marching along y or z over a chunk of
+//                        cells.  The five-cell reconstruction window of the column lives in a
+//                        thread-private shared-memory ring (no __syncthreads anywhere); the high face
+//                        state and the low-face flux of the previous cell stay in registers.
+//                        MODE 1 (y): D = D + dF_y.   MODE 2 (z): out = RK stage update with
+//                        (D + dF_z), i.e. the paper's sum order ((dFx + dFy) + dFz).
+//
+// `PH` is the physics policy (k_sweep.cu): NV reconstructed variables, SW_NR window variables per
+// cell (the last one may be a face auxiliary such as kappa_R rho), `states` = limited face states of
+// one cell, `flux<DIR>` = Riemann flux through a face.  Each face state / face of the grid is counted
+// by exactly one thread for the integer diagnostics (same convention as the oracle: states of the
+// cells -1..n and faces 0..n of the sweep direction, other two indices interior).
+#pragma once
+
+#include "k_stage_common.cuh"
+
+namespace qk {
+
+constexpr int SW_NT = 128;    // threads per CTA of the marching kernels (lanes along x)
+constexpr int SW_NR = 5;      // variables per cell kept in the marching window
+constexpr int SW_XW = 30;     // cells updated per warp in the x sweep
+constexpr int SW_XROWS = 4;   // rows (warps) per CTA in the x sweep
+
+template <int NV> struct FieldsRW { double *f[NV]; };
+template <int NV> struct FieldsRO { const double *f[NV]; };
+
+struct RkArgs { double dtdx; int stage; };
+
+__device__ __forceinline__ void sweep_count(Counters *ctr, int nfall, int nguard)
+{
+    for (int off = 16; off > 0; off >>= 1) {
+        nfall += __shfl_xor_sync(0xffffffffu, nfall, off);
+        nguard += __shfl_xor_sync(0xffffffffu, nguard, off);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        if (nfall) atomicAdd((unsigned long long *)&ctr->fallback, (unsigned long long)nfall);
+        if (nguard) atomicAdd((unsigned long long *)&ctr->guard, (unsigned long long)nguard);
+    }
+}
+
+template <class PH>
+__global__ void __launch_bounds__(32 * SW_XROWS) sweep_x_kernel(PH ph, Geom g, FieldsRW<PH::NV> D, Counters *ctr)
+{
+    constexpr int NV = PH::NV;
+    constexpr unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x;
+    const int j = blockIdx.y * SW_XROWS + threadIdx.y, k = blockIdx.z;
+    int nfall = 0, nguard = 0;
+    if (j < g.ny) {     // warp-uniform
+        const int i = (int)blockIdx.x * SW_XW - 1 + lane;
+        const int cidx = g.at(min(i, g.nx), j, k);      // lanes beyond cell n repeat cell n (not stored, not counted)
+        double lo[NV], hi[NV], L[NV], F[NV];
+        const int nf = ph.states([&](int v, int m) { return ph.ld(v, cidx + m - 2); }, ph.aux(cidx), lo, hi);
+#pragma unroll
+        for (int v = 0; v < NV; ++v) L[v] = __shfl_up_sync(FULL, hi[v], 1);
+        const int gd = ph.template flux<0>(L, lo, ph.ld(SW_NR - 1, cidx - 1), ph.ld(SW_NR - 1, cidx), F);   // face i-1/2
+        const bool interior = lane >= 1 && lane <= SW_XW && i < g.nx;
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+            const double Fh = __shfl_down_sync(FULL, F[v], 1);
+            if (interior) D.f[v][cidx] = Fh - F[v];
+        }
+        if (PH::COUNTS) {
+            const bool last = lane >= 1 && i == g.nx;
+            if (interior || i == -1 || last) nfall = nf;
+            if (interior || last) nguard = gd;
+        }
+    }
+    if (PH::COUNTS) sweep_count(ctr, nfall, nguard);
+}
+
+// DIR = 1 (march along y; blockIdx.y = k) or 2 (march along z; blockIdx.y = j)
+template <class PH, int DIR, int MODE>
+__global__ void __launch_bounds__(SW_NT) sweep_march_kernel(PH ph, Geom g, int len, FieldsRW<PH::NV> D, RkArgs rk,
+                                                            FieldsRO<PH::NV> U, FieldsRO<PH::NV> U0,
+                                                            FieldsRW<PH::NV> out, Counters *ctr)
+{
+    constexpr int NV = PH::NV;
+    __shared__ double ring[5 * SW_NR * SW_NT];          // [slot][var][thread], thread-private columns
+    const int tid = threadIdx.x;
+    const int i = blockIdx.x * SW_NT + tid;
+    const bool active = i < g.nx;
+    const int o = blockIdx.y;
+    const int n_m = DIR == 1 ? g.ny : g.nz;
+    const int m0 = (int)blockIdx.z * len;
+    const int m1 = min(m0 + len, n_m);
+    const int s = DIR == 1 ? g.sy : g.sz;
+    const int ic = min(i, g.nx - 1);
+    const int base = DIR == 1 ? g.at(ic, 0, o) : g.at(ic, o, 0);     // cell m = 0 of the column
+
+    // rotating ring offsets of the cells m-1, m, m+1, m+2, m+3
+    int r0 = 0 * SW_NR * SW_NT + tid, r1 = 1 * SW_NR * SW_NT + tid, r2 = 2 * SW_NR * SW_NT + tid,
+        r3 = 3 * SW_NR * SW_NT + tid, r4 = 4 * SW_NR * SW_NT + tid;
+    // prologue: cells m0-3..m0 -> r0..r3 (they are cells m-1..m+2 of the first step m = m0-2)
+    {
+        const int rr[4] = {r0, r1, r2, r3};
+#pragma unroll
+        for (int p = 0; p < 4; ++p) {
+            const int cidx = base + (m0 - 3 + p) * s;
+#pragma unroll
+            for (int v = 0; v < SW_NR; ++v) ring[rr[p] + v * SW_NT] = ph.ld(v, cidx);
+        }
+    }
+    double pend[SW_NR];
+#pragma unroll
+    for (int v = 0; v < SW_NR; ++v) pend[v] = ph.ld(v, base + (m0 + 1) * s);
+    double aux_next = ph.aux(base + (m0 - 1) * s);
+    double hiP[NV], Flo[NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) { hiP[v] = 0.0; Flo[v] = 0.0; }
+    int nfall = 0, nguard = 0;
+
+    for (int m = m0 - 2; m < m1; ++m) {
+#pragma unroll
+        for (int v = 0; v < SW_NR; ++v) ring[r4 + v * SW_NT] = pend[v];
+        const double aux = aux_next;
+        if (m + 1 < m1) {
+            const int cn = base + (m + 4) * s;
+#pragma unroll
+            for (int v = 0; v < SW_NR; ++v) pend[v] = ph.ld(v, cn);
+            aux_next = ph.aux(base + (m + 2) * s);
+        }
+        const int cidx = base + m * s;
+        // own-cell inputs of the update, consumed at the end of the step
+        double din[NV], u[NV], u0[NV];
+        if (m >= m0) {
+#pragma unroll
+            for (int v = 0; v < NV; ++v) {
+                din[v] = D.f[v][cidx];
+                if (MODE == 2) {
+                    u[v] = U.f[v][cidx];
+                    u0[v] = rk.stage == 1 ? U0.f[v][cidx] : 0.0;
+                }
+            }
+        }
+        // limited face states of cell m+1
+        double lo[NV], hi[NV], Fhi[NV];
+        {
+            const int rr[5] = {r0, r1, r2, r3, r4};
+            const int nf = ph.states([&](int v, int q) { return ring[rr[q] + v * SW_NT]; }, aux, lo, hi);
+            const int mm = m + 1;
+            if (PH::COUNTS && active && ((mm >= m0 && mm < m1) || mm == -1 || mm == n_m)) nfall += nf;
+        }
+        if (m >= m0 - 1) {      // face m+1/2 = low face of cell m+1
+            const int gd = ph.template flux<DIR>(hiP, lo, ring[r1 + (SW_NR - 1) * SW_NT], ring[r2 + (SW_NR - 1) * SW_NT], Fhi);
+            const int mm = m + 1;
+            if (PH::COUNTS && active && ((mm >= m0 && mm < m1) || mm == n_m)) nguard += gd;
+        }
+        if (m >= m0 && active) {
+#pragma unroll
+            for (int v = 0; v < NV; ++v) {
+                const double div = din[v] + (Fhi[v] - Flo[v]);
+                if (MODE == 1) {
+                    D.f[v][cidx] = div;
+                } else {
+                    const double us = u[v] - rk.dtdx * div;
+                    out.f[v][cidx] = rk.stage == 0 ? us : 0.5 * u0[v] + 0.5 * us;
+                }
+            }
+        }
+#pragma unroll
+        for (int v = 0; v < NV; ++v) { hiP[v] = hi[v]; Flo[v] = Fhi[v]; }
+        const int t = r0; r0 = r1; r1 = r2; r2 = r3; r3 = r4; r4 = t;
+    }
+    if (PH::COUNTS) sweep_count(ctr, nfall, nguard);
+}
+
+}  // namespace qk

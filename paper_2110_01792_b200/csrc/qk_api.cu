@@ -187,18 +187,36 @@ void hydro_stage_fused(qk_ctx *c, double dtdx, int stage, double *const *U, doub
     }
 }
 
+void hydro_stage_sweep(qk_ctx *c, double dtdx, int stage, double *const *U, double *const *U0, double *const *out)
+{
+    const Geom &g = c->g;
+    double *const *W = &c->scratch[0];
+    double *const *D = &c->scratch[5];
+    { Scope s(c, K_PRIM); s.done(launch_prim(g, c->pc.gamma, ch5(U), h5(W), c->ctr, c->stream)); }
+    { Scope s(c, K_FLATTEN); s.done(launch_flatten(g, c->pc.gamma, ch5(W), c->chi, c->stream)); }
+    for (int d = 0; d < 3; ++d) {
+        Scope s(c, K_HYDRO_SWEEP_X + d);
+        s.done(launch_hydro_sweeps(g, c->pc.gamma, dtdx, stage, ch5(W), c->chi, h5(D), ch5(U), ch5(U0), h5(out), c->ctr,
+                                   c->stream, 1 << d));
+    }
+}
+
+void hydro_stage(qk_ctx *c, double dtdx, int stage, double *const *U, double *const *U0, double *const *out)
+{
+    if (c->path == QK_PATH_FUSED) hydro_stage_fused(c, dtdx, stage, U, U0, out);
+    else if (c->path == QK_PATH_SWEEP) hydro_stage_sweep(c, dtdx, stage, U, U0, out);
+    else hydro_stage_unfused(c, dtdx, stage, U, U0, out);
+}
+
 int do_hydro_step(qk_ctx *c, double dt)
 {
     const double dtdx = dt / c->pc.dx;
     double *const *Un = &c->state[QK_RHO];
     double *const *U1 = &c->stage[0];
-    const bool fused = c->path == QK_PATH_FUSED;
     fill_fields(c, Un, 5);
-    if (fused) hydro_stage_fused(c, dtdx, 0, Un, Un, U1);
-    else       hydro_stage_unfused(c, dtdx, 0, Un, Un, U1);
+    hydro_stage(c, dtdx, 0, Un, Un, U1);
     fill_fields(c, U1, 5);
-    if (fused) hydro_stage_fused(c, dtdx, 1, U1, Un, Un);
-    else       hydro_stage_unfused(c, dtdx, 1, U1, Un, Un);
+    hydro_stage(c, dtdx, 1, U1, Un, Un);
     return check_launch();
 }
 
@@ -230,6 +248,26 @@ void rad_stage_fused(qk_ctx *c, double dtdx, int stage, double *const *R, double
                             c->ctr, c->stream));
 }
 
+void rad_stage_sweep(qk_ctx *c, double dtdx, int stage, double *const *R, double *const *R0, double *const *out)
+{
+    const Geom &g = c->g;
+    double *const *S = &c->scratch[0];
+    double *const *D = &c->scratch[5];
+    { Scope s(c, K_RAD_PRIM); s.done(launch_rad_prim(g, c->pc.c, cr4(R), r4(S), c->ctr, c->stream)); }
+    for (int d = 0; d < 3; ++d) {
+        Scope s(c, K_RAD_SWEEP_X + d);
+        s.done(launch_rad_sweeps(g, c->pc, dtdx, stage, cr4(S), c->state[QK_RHO], c->state[QK_KAPPA_R], r4(D), cr4(R),
+                                 cr4(R0), r4(out), c->ctr, c->stream, 1 << d));
+    }
+}
+
+void rad_stage(qk_ctx *c, double dtdx, int stage, double *const *R, double *const *R0, double *const *out)
+{
+    if (c->path == QK_PATH_FUSED) rad_stage_fused(c, dtdx, stage, R, R0, out);
+    else if (c->path == QK_PATH_SWEEP) rad_stage_sweep(c, dtdx, stage, R, R0, out);
+    else rad_stage_unfused(c, dtdx, stage, R, R0, out);
+}
+
 int do_rad_transport(qk_ctx *c, double dt)
 {
     const double dtdx = dt / c->pc.dx;
@@ -237,13 +275,10 @@ int do_rad_transport(qk_ctx *c, double dt)
     double *const *R1 = &c->stage[0];
     // rho and kappa_R ghosts feed tau_face at the domain faces
     double *first[6] = {Rn[0], Rn[1], Rn[2], Rn[3], c->state[QK_RHO], c->state[QK_KAPPA_R]};
-    const bool fused = c->path == QK_PATH_FUSED;
     fill_fields(c, first, 6);
-    if (fused) rad_stage_fused(c, dtdx, 0, Rn, Rn, R1);
-    else       rad_stage_unfused(c, dtdx, 0, Rn, Rn, R1);
+    rad_stage(c, dtdx, 0, Rn, Rn, R1);
     fill_fields(c, R1, 4);
-    if (fused) rad_stage_fused(c, dtdx, 1, R1, Rn, Rn);
-    else       rad_stage_unfused(c, dtdx, 1, R1, Rn, Rn);
+    rad_stage(c, dtdx, 1, R1, Rn, Rn);
     return check_launch();
 }
 
@@ -347,7 +382,7 @@ int qk_set_params(qk_ctx *c, double cfl, double newton_tol, int newton_maxit, in
 
 int qk_set_path(qk_ctx *c, int path)
 {
-    if (!c || (path != QK_PATH_FUSED && path != QK_PATH_UNFUSED)) return QK_EINVAL;
+    if (!c || path < QK_PATH_FUSED || path > QK_PATH_SWEEP) return QK_EINVAL;
     c->path = path;
     return QK_OK;
 }
@@ -532,7 +567,9 @@ int qk_kernel_class_count(void) { return K_NCLASS; }
 const char *qk_kernel_class_name(int cls)
 {
     static const char *names[K_NCLASS] = {"fill_boundary", "cfl", "prim", "flatten", "hydro_flux", "hydro_update",
-                                          "hydro_stage", "rad_prim", "rad_flux", "rad_update", "rad_stage", "exchange"};
+                                          "hydro_stage", "rad_prim", "rad_flux", "rad_update", "rad_stage", "exchange",
+                                          "hydro_sweep_x", "hydro_sweep_y", "hydro_sweep_z", "rad_sweep_x",
+                                          "rad_sweep_y", "rad_sweep_z"};
     return (cls >= 0 && cls < K_NCLASS) ? names[cls] : "";
 }
 

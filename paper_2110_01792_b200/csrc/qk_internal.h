@@ -46,7 +46,9 @@ struct Counters {
 
 // Kernel classes for per-kernel timing (qk_kernel_times) -- one id per __global__ function family.
 enum KClass { K_FILL = 0, K_CFL, K_PRIM, K_FLATTEN, K_HYDRO_FLUX, K_HYDRO_UPDATE, K_HYDRO_STAGE,
-              K_RAD_PRIM, K_RAD_FLUX, K_RAD_UPDATE, K_RAD_STAGE, K_EXCHANGE, K_NCLASS };
+              K_RAD_PRIM, K_RAD_FLUX, K_RAD_UPDATE, K_RAD_STAGE, K_EXCHANGE,
+              K_HYDRO_SWEEP_X, K_HYDRO_SWEEP_Y, K_HYDRO_SWEEP_Z, K_RAD_SWEEP_X, K_RAD_SWEEP_Y, K_RAD_SWEEP_Z,
+              K_NCLASS };
 
 struct PhysConsts {
     double dx, gamma, c_hat, c, a_rad, kB_mu, cfl, newton_tol;
@@ -80,6 +82,13 @@ int launch_hydro_stage(const Geom &g, double gamma, double dtdx, int stage, CHyd
 
 int launch_rad_stage(const Geom &g, const PhysConsts &pc, double dtdx, int stage, CRad4p R, CRad4p R0, const double *rho,
                      const double *kappaR, Rad4p out, Counters *ctr, cudaStream_t st);
+
+// sweep path (k_sweep.cu); `which` bit 0 = x sweep, bit 1 = y sweep, bit 2 = z sweep + RK update
+int launch_hydro_sweeps(const Geom &g, double gamma, double dtdx, int stage, CHydro5 W, const double *chi, Hydro5 D,
+                        CHydro5 U, CHydro5 U0, Hydro5 out, Counters *ctr, cudaStream_t st, int which);
+int launch_rad_sweeps(const Geom &g, const PhysConsts &pc, double dtdx, int stage, CRad4p S, const double *rho,
+                      const double *kappaR, Rad4p D, CRad4p R, CRad4p R0, Rad4p out, Counters *ctr, cudaStream_t st,
+                      int which);
 
 int launch_rad_prim(const Geom &g, double c, CRad4p R, Rad4p S, Counters *ctr, cudaStream_t st);
 int launch_rad_flux(const Geom &g, const PhysConsts &pc, int dir, CRad4p S, const double *rho, const double *kappaR,

@@ -14,8 +14,8 @@ import parity_util as P
 
 pytestmark = pytest.mark.gpu
 
-PATHS = [B.QK_PATH_FUSED, B.QK_PATH_UNFUSED]
-PATH_IDS = ["fused", "unfused"]
+PATHS = [B.QK_PATH_FUSED, B.QK_PATH_UNFUSED, B.QK_PATH_SWEEP]
+PATH_IDS = ["fused", "unfused", "sweep"]
 
 
 # ------------------------------------------------------------------------------------------------
