@@ -59,6 +59,47 @@ struct RadPh {
     }
 };
 
+// ---- flattening coefficient in two pointwise passes (H6) -------------------------------
+// pass 1: chi~_x, chi~_y, chi~_z of every cell of [-2, n+1]^3 (one evaluation per cell and direction);
+// pass 2: chi = min over the three directions and the -1, 0, +1 neighbours along each, cells [-1, n]^3.
+__global__ void __launch_bounds__(128) chi_dir_kernel(Geom g, double gamma, const double *__restrict__ P,
+                                                      const double *__restrict__ vx, const double *__restrict__ vy,
+                                                      const double *__restrict__ vz, double *__restrict__ cx,
+                                                      double *__restrict__ cy, double *__restrict__ cz)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x - 2;
+    const int j = (int)blockIdx.y - 2, k = (int)blockIdx.z - 2;
+    if (i > g.nx + 1) return;
+    const int c = g.at(i, j, k), sy = g.sy, sz = g.sz;
+    const double P0 = P[c];
+    cx[c] = flatten_coeff_1d(gamma, P[c - 2], P[c - 1], P0, P[c + 1], P[c + 2], vx[c - 1], vx[c + 1]);
+    cy[c] = flatten_coeff_1d(gamma, P[c - 2 * sy], P[c - sy], P0, P[c + sy], P[c + 2 * sy], vy[c - sy], vy[c + sy]);
+    cz[c] = flatten_coeff_1d(gamma, P[c - 2 * sz], P[c - sz], P0, P[c + sz], P[c + 2 * sz], vz[c - sz], vz[c + sz]);
+}
+
+__global__ void __launch_bounds__(128) chi_min_kernel(Geom g, const double *__restrict__ cx, const double *__restrict__ cy,
+                                                      const double *__restrict__ cz, double *__restrict__ chi)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x - 1;
+    const int j = (int)blockIdx.y - 1, k = (int)blockIdx.z - 1;
+    if (i > g.nx) return;
+    const int c = g.at(i, j, k), sy = g.sy, sz = g.sz;
+    double x = 1.0;      // same nesting as the oracle: min(1, min(lo, min(mid, hi))) per direction
+    x = lesser(x, lesser(cx[c - 1], lesser(cx[c], cx[c + 1])));
+    x = lesser(x, lesser(cy[c - sy], lesser(cy[c], cy[c + sy])));
+    x = lesser(x, lesser(cz[c - sz], lesser(cz[c], cz[c + sz])));
+    chi[c] = x;
+}
+
+int launch_chi_two_pass(const Geom &g, double gamma, CHydro5 W, double *cx, double *cy, double *cz, double *chi,
+                        cudaStream_t st)
+{
+    dim3 g1((g.nx + 4 + 127) / 128, g.ny + 4, g.nz + 4), g2((g.nx + 2 + 127) / 128, g.ny + 2, g.nz + 2);
+    chi_dir_kernel<<<g1, 128, 0, st>>>(g, gamma, W.E, W.mx, W.my, W.mz, cx, cy, cz);
+    chi_min_kernel<<<g2, 128, 0, st>>>(g, cx, cy, cz, chi);
+    return 2;
+}
+
 static int sweep_len(int n_m, long long columns)
 {
     static int forced = -1;

@@ -81,7 +81,7 @@ __global__ void __launch_bounds__(32 * SW_XROWS) sweep_x_kernel(PH ph, Geom g, F
 
 // DIR = 1 (march along y; blockIdx.y = k) or 2 (march along z; blockIdx.y = j)
 template <class PH, int DIR, int MODE>
-__global__ void __launch_bounds__(SW_NT) sweep_march_kernel(PH ph, Geom g, int len, FieldsRW<PH::NV> D, RkArgs rk,
+__global__ void __launch_bounds__(SW_NT, MODE == 2 ? 3 : 4) sweep_march_kernel(PH ph, Geom g, int len, FieldsRW<PH::NV> D, RkArgs rk,
                                                             FieldsRO<PH::NV> U, FieldsRO<PH::NV> U0,
                                                             FieldsRW<PH::NV> out, Counters *ctr)
 {

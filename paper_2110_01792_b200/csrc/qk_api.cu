@@ -193,7 +193,11 @@ void hydro_stage_sweep(qk_ctx *c, double dtdx, int stage, double *const *U, doub
     double *const *W = &c->scratch[0];
     double *const *D = &c->scratch[5];
     { Scope s(c, K_PRIM); s.done(launch_prim(g, c->pc.gamma, ch5(U), h5(W), c->ctr, c->stream)); }
-    { Scope s(c, K_FLATTEN); s.done(launch_flatten(g, c->pc.gamma, ch5(W), c->chi, c->stream)); }
+    {
+        Scope s(c, K_FLATTEN);
+        s.done(launch_chi_two_pass(g, c->pc.gamma, ch5(W), c->scratch[10], c->scratch[11], c->scratch[12], c->chi,
+                                   c->stream));
+    }
     for (int d = 0; d < 3; ++d) {
         Scope s(c, K_HYDRO_SWEEP_X + d);
         s.done(launch_hydro_sweeps(g, c->pc.gamma, dtdx, stage, ch5(W), c->chi, h5(D), ch5(U), ch5(U0), h5(out), c->ctr,
