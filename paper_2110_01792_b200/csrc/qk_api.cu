@@ -330,7 +330,7 @@ int qk_init(int nx, int ny, int nz, double dx, double gamma, double c_hat, doubl
     x->pc.a_rad = 1.0; x->pc.kB_mu = 1.0; x->pc.cfl = 0.3; x->pc.newton_tol = 1e-10;
     x->pc.newton_maxit = 400; x->pc.nsub_max = 10; x->pc.flags = QK_FLAG_TAU_CORR; x->pc.bc = boundary;
     x->stream = nullptr; x->device = dev; x->base = nullptr; x->bytes = 0; x->owns = false; x->ready = false;
-    x->path = QK_PATH_FUSED; x->launches = 0; x->last_nsub = 0; x->profiling = false;
+    x->path = QK_PATH_SWEEP; x->launches = 0; x->last_nsub = 0; x->profiling = false;
     *out = x;
     return QK_OK;
 }

@@ -132,7 +132,7 @@ def test_hydro_config1_one_and_ten_steps(path):
 
 def test_hydro_config1_hundred_steps():
     params, fields = I.config1()
-    res = _run_hydro_pair(params, fields, 100, B.QK_PATH_FUSED)
+    res = _run_hydro_pair(params, fields, 100, B.QK_PATH_SWEEP)
     errs = P.assert_parity(*res[100], P.TOL_100_STEPS, P.HYDRO, "config1 step 100")
     print("config1, 100 steps, rel errors:", errs)
 
@@ -152,7 +152,7 @@ def test_hydro_ragged_shocks(bc, path):
 def test_hydro_thin_and_tiny_boxes(shape):
     """Degenerate extents (1-3 cells across, where periodic ghosts wrap several times)."""
     params, fields = I.ragged_hydro(shape=shape, seed=5)
-    res = _run_hydro_pair(params, fields, 3, B.QK_PATH_FUSED, check_at=(1,))
+    res = _run_hydro_pair(params, fields, 3, B.QK_PATH_SWEEP, check_at=(1,))
     P.assert_parity(*res[1], P.TOL_ONE_STEP, P.HYDRO, "thin %s" % (shape,))
     P.assert_parity(*res[3], P.TOL_100_STEPS, P.HYDRO, "thin %s" % (shape,))
 
@@ -160,7 +160,7 @@ def test_hydro_thin_and_tiny_boxes(shape):
 def test_hydro_sedov_small_bitwise():
     """The paper's hydro benchmark problem at 40^3: strong shock from rest."""
     params, fields = I.sedov(n=40)
-    res = _run_hydro_pair(params, fields, 8, B.QK_PATH_FUSED)
+    res = _run_hydro_pair(params, fields, 8, B.QK_PATH_SWEEP)
     P.assert_parity(*res[8], P.TOL_100_STEPS, P.HYDRO, "sedov")
     print("sedov mismatching cells:", P.count_mismatch(*res[8], I.FIELDS[:5]))
 
