@@ -164,6 +164,14 @@ int qk_kernel_times(qk_ctx *ctx, double *ms, long long *count);
  * kind 1 = DFMA chains.  Writes fp64 instructions x 32 lanes per second.  Synchronises. */
 int qk_fp64_probe(int kind, int iters, void *cuda_stream, double *lane_ops_per_s);
 
+/* Self-test of the library's branch-free fp64 division and square root (used inside the Riemann
+ * solvers of the sweep kernels): n seeded random operand pairs with exponents
+ * spread over `exponent_span` binades centred on 1 (2046 = every normal double; zeros, subnormals,
+ * infinities and NaNs are mixed in).  out4 = {divisions accepted by the range test, of those not
+ * bit-equal to IEEE x/y, square roots accepted, of those not bit-equal to IEEE sqrt}.  Synchronises. */
+int qk_selftest_divsqrt(long long n, unsigned long long seed, int exponent_span, void *cuda_stream,
+                        long long *out4);
+
 const char *qk_version(void);
 
 #ifdef __cplusplus

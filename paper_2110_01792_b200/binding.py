@@ -28,6 +28,7 @@ EXPORTS = [
     "qk_cfl_dt", "qk_hydro_step", "qk_rad_transport", "qk_exchange", "qk_rad_step", "qk_rhd_step",
     "qk_nsub_for", "qk_last_info", "qk_launch_count", "qk_set_path", "qk_set_profiling",
     "qk_kernel_class_count", "qk_kernel_class_name", "qk_kernel_times", "qk_version", "qk_fp64_probe",
+    "qk_selftest_divsqrt",
 ]
 
 
@@ -83,6 +84,7 @@ def lib():
         "qk_kernel_times": (i, [p, C.POINTER(d), C.POINTER(ll)]),
         "qk_version": (C.c_char_p, []),
         "qk_fp64_probe": (i, [i, i, p, C.POINTER(d)]),
+        "qk_selftest_divsqrt": (i, [ll, C.c_ulonglong, i, p, C.POINTER(ll)]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)
@@ -99,6 +101,15 @@ def qk_fp64_probe(kind=0, iters=20000):
     _check(lib().qk_fp64_probe(kind, iters, C.c_void_p(torch.cuda.current_stream().cuda_stream), C.byref(out)),
            "qk_fp64_probe")
     return float(out.value)
+
+
+def qk_selftest_divsqrt(n, seed=1, exponent_span=2046):
+    """(div accepted, div mismatches, sqrt accepted, sqrt mismatches) -- see include/qk.h."""
+    import torch
+    out = (C.c_longlong * 4)()
+    _check(lib().qk_selftest_divsqrt(n, seed, exponent_span, C.c_void_p(torch.cuda.current_stream().cuda_stream), out),
+           "qk_selftest_divsqrt")
+    return tuple(int(v) for v in out)
 
 
 def _check(rc, what):

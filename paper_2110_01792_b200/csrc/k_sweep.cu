@@ -6,28 +6,74 @@
 #include <stdlib.h>
 
 #include "k_sweep.cuh"
+#include "qk_fastmath.cuh"
+
+#ifndef QK_BLX_H
+#define QK_BLX_H 1
+#endif
+#ifndef QK_BLM_H
+#define QK_BLM_H 0
+#endif
+#ifndef QK_BLX_R
+#define QK_BLX_R 1
+#endif
+#ifndef QK_BLM_R
+#define QK_BLM_R 1
+#endif
 
 namespace qk {
+
+// Out-of-line plain-operator versions of the face fluxes: taken only by the faces whose operands left
+// the range in which the branch-free division / square root of qk_fastmath.cuh are exact.
+__device__ __noinline__ Flux5 hllc_flux_slow(double gamma, double rL, double uL, double vL, double wL, double pL,
+                                             double rR, double uR, double vR, double wR, double pR)
+{
+    return hllc_flux(gamma, rL, uL, vL, wL, pL, rR, uR, vR, wR, pR);
+}
+
+__device__ __noinline__ Rad4 rad_hll_flux_slow(double c, double c_hat, double EL, double fxL, double fyL, double fzL,
+                                               double ER, double fxR, double fyR, double fzR, int n, double tau,
+                                               bool tau_corr, int *guard)
+{
+    int gd;
+    const Rad4 G = rad_hll_flux(c, c_hat, EL, fxL, fyL, fzL, ER, fxR, fyR, fzR, n, tau, tau_corr, gd);
+    *guard = gd;
+    return G;
+}
 
 // ---- hydro ------------------------------------------------------------------------------------------
 struct HydroPh {
     static constexpr int NV = 5;
     static constexpr bool COUNTS = false;
+    // select-only PPM limiter (same values): measured faster in the x sweep, slower in the marching sweeps
+    static constexpr int BL_X = QK_BLX_H, BL_MARCH = QK_BLM_H;   // 0 branches, 1 selects, 2 selects in lockstep
     const double *w[5];        // rho, vx, vy, vz, P (ghost cells included)
     const double *chi;         // flattening coefficient of the cells -1..n
     double gamma;
     __device__ __forceinline__ double ld(int v, int cidx) const { return __ldg(w[v] + cidx); }
     __device__ __forceinline__ double aux(int cidx) const { return __ldg(chi + cidx); }
-    template <class Q>
+    // x sweep: staged sources 0..4 = W, 5 = chi
+    __device__ __forceinline__ const double *src(int s) const { return s < 5 ? w[s] : chi; }
+    __device__ __forceinline__ double win(int v, const double (*buf)[SW_XSEG], int p) const { return buf[v][p]; }
+    __device__ __forceinline__ double win_aux(const double (*buf)[SW_XSEG], int p) const { return buf[5][p]; }
+    template <int BL, class Q>
     __device__ __forceinline__ int states(Q q, double x, double lo[5], double hi[5]) const
     {
-        ppm_cell(q, x, lo, hi);
+        ppm_cell<BL>(q, x, lo, hi);
         return 0;
     }
     template <int DIR>
     __device__ __forceinline__ int flux(const double L[5], const double R[5], double, double, double F[5]) const
     {
+#ifdef QK_PLAIN_DIVSQRT
         face_flux<DIR>(gamma, L, R, F);
+#else
+        constexpr int n = 1 + DIR, t1 = 1 + (DIR + 1) % 3, t2 = 1 + (DIR + 2) % 3;
+        unsigned risk = 0;
+        Flux5 f = hllc_flux_fast(gamma, L[0], L[n], L[t1], L[t2], L[4], R[0], R[n], R[t1], R[t2], R[4], risk);
+        if (risk) f = hllc_flux_slow(gamma, L[0], L[n], L[t1], L[t2], L[4], R[0], R[n], R[t1], R[t2], R[4]);
+        F[0] = f.m; F[n] = f.pn; F[t1] = f.pt1; F[t2] = f.pt2; F[4] = f.e;
+#endif
         return 0;
     }
 };
@@ -36,6 +82,7 @@ struct HydroPh {
 struct RadPh {
     static constexpr int NV = 4;
     static constexpr bool COUNTS = true;
+    static constexpr int BL_X = QK_BLX_R, BL_MARCH = QK_BLM_R;
     const double *s[4];        // E_r, fx, fy, fz
     const double *rho, *kR;
     double c, c_hat, dx;
@@ -46,16 +93,34 @@ struct RadPh {
         return __ldg(kR + cidx) * __ldg(rho + cidx);      // kappa_R rho of the cell
     }
     __device__ __forceinline__ double aux(int) const { return 0.0; }
-    template <class Q>
+    // x sweep: staged sources 0..3 = S, 4 = kappa_R, 5 = rho
+    __device__ __forceinline__ const double *src(int i) const { return i < 4 ? s[i] : (i == 4 ? kR : rho); }
+    __device__ __forceinline__ double win(int v, const double (*buf)[SW_XSEG], int p) const
+    {
+        return v < 4 ? buf[v][p] : buf[4][p] * buf[5][p];
+    }
+    __device__ __forceinline__ double win_aux(const double (*)[SW_XSEG], int) const { return 0.0; }
+    template <int BL, class Q>
     __device__ __forceinline__ int states(Q q, double, double lo[4], double hi[4]) const
     {
-        return rad_ppm_cell(q, lo, hi);
+        return rad_ppm_cell<BL>(q, lo, hi);
     }
     template <int DIR>
     __device__ __forceinline__ int flux(const double L[4], const double R[4], double krL, double krR, double G[4]) const
     {
         const double tau = (0.5 * (krL + krR)) * dx;
+#ifdef QK_PLAIN_DIVSQRT
         return rad_face_flux<DIR>(c, c_hat, tau_corr != 0, tau, L, R, G);
+#else
+        unsigned risk = 0;
+        int guard;
+        Rad4 g = rad_hll_flux_fast(c, c_hat, L[0], L[1], L[2], L[3], R[0], R[1], R[2], R[3], DIR, tau, tau_corr != 0,
+                                   guard, risk);
+        if (risk) g = rad_hll_flux_slow(c, c_hat, L[0], L[1], L[2], L[3], R[0], R[1], R[2], R[3], DIR, tau,
+                                        tau_corr != 0, &guard);
+        G[0] = g.e; G[1] = g.x; G[2] = g.y; G[3] = g.z;
+        return guard;
+#endif
     }
 };
 
@@ -121,7 +186,8 @@ static int launch_sweeps(const PH &ph, const Geom &g, double dtdx, int stage, Fi
     const RkArgs rk{dtdx, stage};
     int n = 0;
     if (which & 1) {
-        dim3 grid((g.nx + SW_XW - 1) / SW_XW, (g.ny + SW_XROWS - 1) / SW_XROWS, g.nz), block(32, SW_XROWS);
+        constexpr int rows = SW_XROWS * SW_XNROW;
+        dim3 grid((g.nx + SW_XW - 1) / SW_XW, (g.ny + rows - 1) / rows, g.nz), block(32, SW_XROWS);
         sweep_x_kernel<PH><<<grid, block, 0, st>>>(ph, g, D, ctr);
         ++n;
     }

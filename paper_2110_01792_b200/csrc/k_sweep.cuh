@@ -26,10 +26,25 @@
 
 namespace qk {
 
-constexpr int SW_NT = 128;    // threads per CTA of the marching kernels (lanes along x)
-constexpr int SW_NR = 5;      // variables per cell kept in the marching window
-constexpr int SW_XW = 30;     // cells updated per warp in the x sweep
-constexpr int SW_XROWS = 4;   // rows (warps) per CTA in the x sweep
+#ifndef QK_SW_NT
+#define QK_SW_NT 128
+#endif
+#ifndef QK_SW_MINB1
+#define QK_SW_MINB1 4
+#endif
+#ifndef QK_SW_MINB2
+#define QK_SW_MINB2 3
+#endif
+#ifndef QK_SW_XROWS
+#define QK_SW_XROWS 4
+#endif
+#ifndef QK_SW_XMINB
+#define QK_SW_XMINB 1
+#endif
+constexpr int SW_NT = QK_SW_NT;       // threads per CTA of the marching kernels (lanes along x)
+constexpr int SW_NR = 5;              // variables per cell kept in the marching window
+constexpr int SW_XW = 30;             // cells updated per warp in the x sweep
+constexpr int SW_XROWS = QK_SW_XROWS; // rows (warps) per CTA in the x sweep
 
 template <int NV> struct FieldsRW { double *f[NV]; };
 template <int NV> struct FieldsRO { const double *f[NV]; };
@@ -48,22 +63,68 @@ __device__ __forceinline__ void sweep_count(Counters *ctr, int nfall, int nguard
     }
 }
 
+// ---- x sweep -------------------------------------------------------------------------------------------
+// Each warp owns one 30-cell x segment and walks SW_XNROW consecutive rows of it.  The 36-cell row
+// segment of every source array the stencils of its 32 lanes touch is copied global -> shared with
+// cp.async (no register staging), one row ahead of the arithmetic, into a warp-private double buffer:
+// the copy of row r+1 overlaps the PPM / Riemann work of row r and the only synchronisation is
+// __syncwarp.  (Loading the stencils straight from global memory exposed one full memory latency per
+// variable: 45 % of the stall samples, profiles/r1_hydro_ncu.md.)
+#ifndef QK_SW_XNROW
+#define QK_SW_XNROW 8
+#endif
+constexpr int SW_XNROW = QK_SW_XNROW;   // rows walked by one warp
+constexpr int SW_XSEG = SW_XW + 6;      // staged cells per row: lanes' cells -1..30 plus the +-2 stencil halo
+constexpr int SW_NSRC = 6;              // source arrays per policy (window variables are built from them)
+
+__device__ __forceinline__ void cp_async8(double *smem_dst, const double *gsrc)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gsrc)
+                 : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
 template <class PH>
-__global__ void __launch_bounds__(32 * SW_XROWS) sweep_x_kernel(PH ph, Geom g, FieldsRW<PH::NV> D, Counters *ctr)
+__global__ void __launch_bounds__(32 * SW_XROWS, QK_SW_XMINB) sweep_x_kernel(PH ph, Geom g, FieldsRW<PH::NV> D, Counters *ctr)
 {
     constexpr int NV = PH::NV;
     constexpr unsigned FULL = 0xffffffffu;
-    const int lane = threadIdx.x;
-    const int j = blockIdx.y * SW_XROWS + threadIdx.y, k = blockIdx.z;
+    __shared__ double stage[SW_XROWS][2][SW_NSRC][SW_XSEG];
+    const int lane = threadIdx.x, wy = threadIdx.y;
+    const int k = blockIdx.z;
+    const int j0 = ((int)blockIdx.y * SW_XROWS + wy) * SW_XNROW;
+    const int i0 = (int)blockIdx.x * SW_XW;
+    const int i = i0 - 1 + lane;                              // this lane's cell
     int nfall = 0, nguard = 0;
-    if (j < g.ny) {     // warp-uniform
-        const int i = (int)blockIdx.x * SW_XW - 1 + lane;
-        const int cidx = g.at(min(i, g.nx), j, k);      // lanes beyond cell n repeat cell n (not stored, not counted)
+    const int nrow = min(SW_XNROW, g.ny - j0);                // warp-uniform; <= 0 for warps past the last row
+
+    // cells staged by this lane: i0-3+lane, and for lanes 0..3 also i0+29+lane (clamped into the array)
+    const int ia = min(i0 - 3 + lane, g.nx + NG - 1), ib = min(i0 + 29 + lane, g.nx + NG - 1);
+    auto issue = [&](int r) {
+        const int rowbase = g.at(0, j0 + r, k);
+        double(*buf)[SW_XSEG] = stage[wy][r & 1];
+#pragma unroll
+        for (int sidx = 0; sidx < SW_NSRC; ++sidx) {
+            const double *src = ph.src(sidx) + rowbase;
+            cp_async8(&buf[sidx][lane], src + ia);
+            if (lane < SW_XSEG - 32) cp_async8(&buf[sidx][32 + lane], src + ib);
+        }
+        cp_async_commit();
+    };
+    if (nrow > 0) issue(0);
+    for (int r = 0; r < nrow; ++r) {
+        if (r + 1 < nrow) { issue(r + 1); cp_async_wait<1>(); }
+        else              { cp_async_wait<0>(); }
+        __syncwarp();
+        const double(*buf)[SW_XSEG] = stage[wy][r & 1];
+        const int cidx = g.at(min(i, g.nx), j0 + r, k);      // lanes beyond cell n are not stored, not counted
         double lo[NV], hi[NV], L[NV], F[NV];
-        const int nf = ph.states([&](int v, int m) { return ph.ld(v, cidx + m - 2); }, ph.aux(cidx), lo, hi);
+        const int nf = ph.template states<PH::BL_X>([&](int v, int m) { return ph.win(v, buf, lane + m); },
+                                                     ph.win_aux(buf, lane + 2), lo, hi);
 #pragma unroll
         for (int v = 0; v < NV; ++v) L[v] = __shfl_up_sync(FULL, hi[v], 1);
-        const int gd = ph.template flux<0>(L, lo, ph.ld(SW_NR - 1, cidx - 1), ph.ld(SW_NR - 1, cidx), F);   // face i-1/2
+        const int gd = ph.template flux<0>(L, lo, ph.win(SW_NR - 1, buf, lane + 1), ph.win(SW_NR - 1, buf, lane + 2), F);   // face i-1/2
         const bool interior = lane >= 1 && lane <= SW_XW && i < g.nx;
 #pragma unroll
         for (int v = 0; v < NV; ++v) {
@@ -72,16 +133,17 @@ __global__ void __launch_bounds__(32 * SW_XROWS) sweep_x_kernel(PH ph, Geom g, F
         }
         if (PH::COUNTS) {
             const bool last = lane >= 1 && i == g.nx;
-            if (interior || i == -1 || last) nfall = nf;
-            if (interior || last) nguard = gd;
+            if (interior || i == -1 || last) nfall += nf;
+            if (interior || last) nguard += gd;
         }
+        __syncwarp();                                         // all lanes done with buf before it is refilled
     }
     if (PH::COUNTS) sweep_count(ctr, nfall, nguard);
 }
 
 // DIR = 1 (march along y; blockIdx.y = k) or 2 (march along z; blockIdx.y = j)
 template <class PH, int DIR, int MODE>
-__global__ void __launch_bounds__(SW_NT, MODE == 2 ? 3 : 4) sweep_march_kernel(PH ph, Geom g, int len, FieldsRW<PH::NV> D, RkArgs rk,
+__global__ void __launch_bounds__(SW_NT, MODE == 2 ? QK_SW_MINB2 : QK_SW_MINB1) sweep_march_kernel(PH ph, Geom g, int len, FieldsRW<PH::NV> D, RkArgs rk,
                                                             FieldsRO<PH::NV> U, FieldsRO<PH::NV> U0,
                                                             FieldsRW<PH::NV> out, Counters *ctr)
 {
@@ -147,7 +209,7 @@ __global__ void __launch_bounds__(SW_NT, MODE == 2 ? 3 : 4) sweep_march_kernel(P
         double lo[NV], hi[NV], Fhi[NV];
         {
             const int rr[5] = {r0, r1, r2, r3, r4};
-            const int nf = ph.states([&](int v, int q) { return ring[rr[q] + v * SW_NT]; }, aux, lo, hi);
+            const int nf = ph.template states<PH::BL_MARCH>([&](int v, int q) { return ring[rr[q] + v * SW_NT]; }, aux, lo, hi);
             const int mm = m + 1;
             if (PH::COUNTS && active && ((mm >= m0 && mm < m1) || mm == -1 || mm == n_m)) nfall += nf;
         }

@@ -58,7 +58,8 @@ QK_HD double mc_slope(double qW, double qC, double qE)
 // eq 22 interface values with mirror-symmetric brackets, three-cell clamp
 // (H3), then the parabola check: extremum -> MC-limited line (H4), one-sided
 // overshoot -> CW84 correction (H5).  qlo = state at j-1/2, qhi = state at j+1/2.
-QK_HD void ppm_face_states(double a, double b, double c, double d, double e, double &qlo, double &qhi)
+template <bool BRANCHLESS>
+QK_HD void ppm_face_states_t(double a, double b, double c, double d, double e, double &qlo, double &qhi)
 {
     const double w7 = 7.0 / 12.0, w1 = 1.0 / 12.0;
     double lo_face = w7 * (b + c) - w1 * (d + a);
@@ -68,6 +69,20 @@ QK_HD void ppm_face_states(double a, double b, double c, double d, double e, dou
     lo_face = lesser(greater(lo_face, floor3), ceil3);
     hi_face = lesser(greater(hi_face, floor3), ceil3);
     const double below = c - lo_face, above = hi_face - c;
+    if (BRANCHLESS) {
+    // same values as the branches below, written as selects so that the variables of a cell
+    // interleave in the fp64 pipe (no divergent control flow)
+    const double s = mc_slope(b, c, d);
+    const bool extremum = below * above <= 0.0;
+    const double ab = fabs(below), aa = fabs(above);
+    const bool fix_lo = ab >= 2.0 * aa;
+    const bool fix_hi = !fix_lo && (aa >= 2.0 * ab);
+    const double lo_fix = c - 2.0 * above, hi_fix = c + 2.0 * below;
+    const double lo_ext = c - 0.5 * s, hi_ext = c + 0.5 * s;
+    qlo = extremum ? lo_ext : (fix_lo ? lo_fix : lo_face);
+    qhi = extremum ? hi_ext : (fix_hi ? hi_fix : hi_face);
+    return;
+    }
     if (below * above <= 0.0) {
         const double s = mc_slope(b, c, d);
         lo_face = c - 0.5 * s;
@@ -79,6 +94,11 @@ QK_HD void ppm_face_states(double a, double b, double c, double d, double e, dou
     }
     qlo = lo_face;
     qhi = hi_face;
+}
+
+QK_HD void ppm_face_states(double a, double b, double c, double d, double e, double &qlo, double &qhi)
+{
+    ppm_face_states_t<false>(a, b, c, d, e, qlo, qhi);
 }
 
 // One-directional shock-flattening coefficient of cell j from the pressures P_{j-2..j+2}

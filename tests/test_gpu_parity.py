@@ -83,6 +83,21 @@ def test_set_get_state_device_pointers():
 
 # ------------------------------------------------------------------------------------------------
 # S2: CFL reduction
+@pytest.mark.parametrize("span", [2046, 600, 40], ids=["all_exponents", "wide", "near_one"])
+def test_fast_div_sqrt_bitwise(span):
+    """The branch-free division / square root inside the sweep kernels' Riemann solvers return the
+    IEEE-rounded result (the bits the oracle's `/` and sqrt() give) for every operand pair their range
+    test accepts; what it rejects is recomputed with the plain operators by the kernels."""
+    n = 1 << 28
+    acc_d, bad_d, acc_s, bad_s = B.qk_selftest_divsqrt(n, seed=12345 + span, exponent_span=span)
+    assert bad_d == 0 and bad_s == 0, (acc_d, bad_d, acc_s, bad_s)
+    # the range test must not be vacuous: near 1 it accepts everything except the injected specials
+    if span == 40:
+        assert acc_d > 0.95 * n and acc_s > 0.95 * n, (acc_d, acc_s)
+    else:
+        assert acc_d > 0.2 * n and acc_s > 0.4 * n, (acc_d, acc_s)
+
+
 # ------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("gen", [lambda: I.config1(), lambda: I.ragged_hydro(), lambda: I.ragged_rhd(),
                                  lambda: I.config2(n=64)], ids=["config1", "ragged", "ragged_rhd", "turb64"])
