@@ -10,7 +10,7 @@
 
 namespace qk {
 
-__global__ void __launch_bounds__(256) cfl_max_speed_kernel(Geom g, double gamma, CHydro5 U, Counters *ctr)
+__global__ void __launch_bounds__(256) cfl_max_speed_kernel(Geom g, double gamma, CHydro5 U, StateCache *ctr)
 {
     const long long ncell = (long long)g.nx * g.ny * g.nz;
     double smax = 0.0;
@@ -49,7 +49,7 @@ __global__ void __launch_bounds__(256) cfl_max_speed_kernel(Geom g, double gamma
     }
 }
 
-int launch_cfl(const Geom &g, double gamma, CHydro5 U, Counters *ctr, cudaStream_t st)
+int launch_cfl(const Geom &g, double gamma, CHydro5 U, StateCache *ctr, cudaStream_t st)
 {
     const long long ncell = (long long)g.nx * g.ny * g.nz;
     long long blocks = (ncell + 255) / 256;

@@ -6,6 +6,7 @@
 // (HBM-bound).  Counters are reduced per warp before the atomics.
 #include "qk_internal.h"
 #include "qk_math.cuh"
+#include "qk_fastmath.cuh"
 
 namespace qk {
 
@@ -15,11 +16,12 @@ __global__ void __launch_bounds__(128) exchange_kernel(Geom g, ExchangeConsts kc
                                                        double *__restrict__ Er, double *__restrict__ Fx,
                                                        double *__restrict__ Fy, double *__restrict__ Fz,
                                                        const double *__restrict__ kP, const double *__restrict__ kR,
-                                                       Counters *ctr)
+                                                       Hydro5 Wout, Rad4p Sout, Counters *ctr, StateCache *cache)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y, k = blockIdx.z;
-    int iters = 0, fail = 0, bad = 0;
+    int iters = 0, fail = 0, bad = 0, bad_hydro = 0;
+    double smax = 0.0;
     if (i < g.nx) {
         const int cidx = g.at(i, j, k);
         double m0 = mx[cidx], m1 = my[cidx], m2 = mz[cidx];
@@ -31,6 +33,18 @@ __global__ void __launch_bounds__(128) exchange_kernel(Geom g, ExchangeConsts kc
         if (!kc.static_matter) { mx[cidx] = m0; my[cidx] = m1; mz[cidx] = m2; }
         E[cidx] = e; Er[cidx] = er;
         Fx[cidx] = f0; Fy[cidx] = f1; Fz[cidx] = f2;
+        if (Wout.rho) {
+            // reconstruction variables of the updated cell for the next hydro / radiation stage and its CFL
+            // speed (same operations as prim_kernel, rad_prim_kernel and cfl_max_speed_kernel)
+            Prim p;
+            double sp;
+            cell_prim_speed(kc.gamma, rho[cidx], m0, m1, m2, e, true, p, sp);
+            Wout.rho[cidx] = p.rho; Wout.mx[cidx] = p.vx; Wout.my[cidx] = p.vy; Wout.mz[cidx] = p.vz; Wout.E[cidx] = p.P;
+            if (!(p.rho > 0.0) || !(p.P > 0.0)) bad_hydro = 1;
+            else smax = sp;
+            const double cE = kc.c * er;
+            Sout.E[cidx] = er; Sout.Fx[cidx] = f0 / cE; Sout.Fy[cidx] = f1 / cE; Sout.Fz[cidx] = f2 / cE;
+        }
     }
     int tot = iters, mxit = iters;
     for (int off = 16; off > 0; off >>= 1) {
@@ -38,18 +52,26 @@ __global__ void __launch_bounds__(128) exchange_kernel(Geom g, ExchangeConsts kc
         mxit = max(mxit, __shfl_xor_sync(0xffffffffu, mxit, off));
         fail += __shfl_xor_sync(0xffffffffu, fail, off);
         bad += __shfl_xor_sync(0xffffffffu, bad, off);
+        bad_hydro += __shfl_xor_sync(0xffffffffu, bad_hydro, off);
+        const double o = __shfl_xor_sync(0xffffffffu, smax, off);
+        if (o > smax) smax = o;
     }
     if ((threadIdx.x & 31) == 0) {
         if (tot) atomicAdd((unsigned long long *)&ctr->newton_total, (unsigned long long)tot);
         if (mxit > 0) atomicMax(&ctr->newton_max, mxit);
         if (fail) atomicAdd((unsigned long long *)&ctr->newton_fail, (unsigned long long)fail);
         if (bad) atomicAdd((unsigned long long *)&ctr->bad_state, (unsigned long long)bad);
+        if (Wout.rho) {
+            const unsigned long long bits = (unsigned long long)__double_as_longlong(smax);
+            if (bits > *(volatile unsigned long long *)&cache->smax_bits) atomicMax(&cache->smax_bits, bits);
+            if (bad_hydro) atomicAdd((unsigned long long *)&cache->cfl_bad, (unsigned long long)bad_hydro);
+        }
     }
 }
 
 int launch_exchange(const Geom &g, const PhysConsts &pc, double dt, const double *rho, double *mx, double *my,
                     double *mz, double *E, double *Er, double *Fx, double *Fy, double *Fz, const double *kP,
-                    const double *kR, Counters *ctr, cudaStream_t st)
+                    const double *kR, Hydro5 Wout, Rad4p Sout, Counters *ctr, StateCache *cache, cudaStream_t st)
 {
     ExchangeConsts kc;
     kc.c = pc.c; kc.c_hat = pc.c_hat; kc.a_rad = pc.a_rad; kc.kB_mu = pc.kB_mu; kc.gamma = pc.gamma;
@@ -57,7 +79,7 @@ int launch_exchange(const Geom &g, const PhysConsts &pc, double dt, const double
     kc.literal_stop = (pc.flags & QK_FLAG_NEWTON_LITERAL) != 0;
     kc.static_matter = (pc.flags & QK_FLAG_STATIC_MATTER) != 0;
     dim3 grid((g.nx + 127) / 128, g.ny, g.nz);
-    exchange_kernel<<<grid, 128, 0, st>>>(g, kc, dt, rho, mx, my, mz, E, Er, Fx, Fy, Fz, kP, kR, ctr);
+    exchange_kernel<<<grid, 128, 0, st>>>(g, kc, dt, rho, mx, my, mz, E, Er, Fx, Fy, Fz, kP, kR, Wout, Sout, ctr, cache);
     return 1;
 }
 

@@ -62,6 +62,39 @@ struct HydroPh {
         ppm_cell<BL>(q, x, lo, hi);
         return 0;
     }
+    // MODE 2 epilogue: primitives of the updated cell for the next stage's sweeps and,
+    // after the last stage, the cell's CFL signal speed |v| + c_s (eq 21), same operations as
+    // prim_kernel / cfl_max_speed_kernel.
+    struct Tail { double smax = 0.0; int bad = 0; };
+    __device__ __forceinline__ void finish(int cidx, const double u[5], const FieldsRW<5> &wout, bool last, Tail &t) const
+    {
+        Prim p;
+        double sp;
+        cell_prim_speed(gamma, u[0], u[1], u[2], u[3], u[4], last, p, sp);
+        wout.f[0][cidx] = p.rho; wout.f[1][cidx] = p.vx; wout.f[2][cidx] = p.vy; wout.f[3][cidx] = p.vz;
+        wout.f[4][cidx] = p.P;
+        if (!(p.rho > 0.0) || !(p.P > 0.0)) { ++t.bad; return; }
+        if (last && sp > t.smax) t.smax = sp;
+    }
+    __device__ __forceinline__ void finish_block(Tail &t, bool last, Counters *ctr, StateCache *cache) const
+    {
+        double smax = t.smax;
+        int bad = t.bad;
+        for (int off = 16; off > 0; off >>= 1) {
+            const double o = __shfl_xor_sync(0xffffffffu, smax, off);
+            if (o > smax) smax = o;
+            bad += __shfl_xor_sync(0xffffffffu, bad, off);
+        }
+        if ((threadIdx.x & 31) == 0) {
+            if (bad) atomicAdd((unsigned long long *)&ctr->bad_state, (unsigned long long)bad);
+            if (last) {
+                const unsigned long long bits = (unsigned long long)__double_as_longlong(smax);
+                // most warps lose against the running maximum: look before paying for the atomic
+                if (bits > *(volatile unsigned long long *)&cache->smax_bits) atomicMax(&cache->smax_bits, bits);
+                if (bad) atomicAdd((unsigned long long *)&cache->cfl_bad, (unsigned long long)bad);
+            }
+        }
+    }
     template <int DIR>
     __device__ __forceinline__ int flux(const double L[5], const double R[5], double, double, double F[5]) const
     {
@@ -104,6 +137,23 @@ struct RadPh {
     __device__ __forceinline__ int states(Q q, double, double lo[4], double hi[4]) const
     {
         return rad_ppm_cell<BL>(q, lo, hi);
+    }
+    // MODE 2 epilogue: (E_r, f = F_r / (c E_r)) of the updated cell, as rad_prim_kernel
+    struct Tail { int bad = 0; };
+    __device__ __forceinline__ void finish(int cidx, const double r[4], const FieldsRW<4> &sout, bool, Tail &t) const
+    {
+        const double cE = c * r[0];
+        sout.f[0][cidx] = r[0];
+        sout.f[1][cidx] = r[1] / cE;
+        sout.f[2][cidx] = r[2] / cE;
+        sout.f[3][cidx] = r[3] / cE;
+        if (!(r[0] > 0.0)) ++t.bad;
+    }
+    __device__ __forceinline__ void finish_block(Tail &t, bool, Counters *ctr, StateCache *) const
+    {
+        int bad = t.bad;
+        for (int off = 16; off > 0; off >>= 1) bad += __shfl_xor_sync(0xffffffffu, bad, off);
+        if ((threadIdx.x & 31) == 0 && bad) atomicAdd((unsigned long long *)&ctr->bad_state, (unsigned long long)bad);
     }
     template <int DIR>
     __device__ __forceinline__ int flux(const double L[4], const double R[4], double krL, double krR, double G[4]) const
@@ -181,7 +231,8 @@ static int sweep_len(int n_m, long long columns)
 
 template <class PH>
 static int launch_sweeps(const PH &ph, const Geom &g, double dtdx, int stage, FieldsRW<PH::NV> D, FieldsRO<PH::NV> U,
-                         FieldsRO<PH::NV> U0, FieldsRW<PH::NV> out, Counters *ctr, cudaStream_t st, int which)
+                         FieldsRO<PH::NV> U0, FieldsRW<PH::NV> out, FieldsRW<PH::NV> pout, Counters *ctr,
+                         StateCache *cache, cudaStream_t st, int which)
 {
     const RkArgs rk{dtdx, stage};
     int n = 0;
@@ -195,32 +246,34 @@ static int launch_sweeps(const PH &ph, const Geom &g, double dtdx, int stage, Fi
     if (which & 2) {
         const int len = sweep_len(g.ny, (long long)g.nx * g.nz);
         dim3 grid(bx, g.nz, (g.ny + len - 1) / len);
-        sweep_march_kernel<PH, 1, 1><<<grid, SW_NT, 0, st>>>(ph, g, len, D, rk, U, U0, out, ctr);
+        sweep_march_kernel<PH, 1, 1><<<grid, SW_NT, 0, st>>>(ph, g, len, D, rk, U, U0, out, pout, ctr, cache);
         ++n;
     }
     if (which & 4) {
         const int len = sweep_len(g.nz, (long long)g.nx * g.ny);
         dim3 grid(bx, g.ny, (g.nz + len - 1) / len);
-        sweep_march_kernel<PH, 2, 2><<<grid, SW_NT, 0, st>>>(ph, g, len, D, rk, U, U0, out, ctr);
+        sweep_march_kernel<PH, 2, 2><<<grid, SW_NT, 0, st>>>(ph, g, len, D, rk, U, U0, out, pout, ctr, cache);
         ++n;
     }
     return n;
 }
 
 int launch_hydro_sweeps(const Geom &g, double gamma, double dtdx, int stage, CHydro5 W, const double *chi, Hydro5 D,
-                        CHydro5 U, CHydro5 U0, Hydro5 out, Counters *ctr, cudaStream_t st, int which)
+                        CHydro5 U, CHydro5 U0, Hydro5 out, Hydro5 Wout, Counters *ctr, StateCache *cache, cudaStream_t st,
+                        int which)
 {
     HydroPh ph;
     ph.w[0] = W.rho; ph.w[1] = W.mx; ph.w[2] = W.my; ph.w[3] = W.mz; ph.w[4] = W.E;
     ph.chi = chi; ph.gamma = gamma;
     FieldsRW<5> d{{D.rho, D.mx, D.my, D.mz, D.E}}, o{{out.rho, out.mx, out.my, out.mz, out.E}};
     FieldsRO<5> u{{U.rho, U.mx, U.my, U.mz, U.E}}, u0{{U0.rho, U0.mx, U0.my, U0.mz, U0.E}};
-    return launch_sweeps(ph, g, dtdx, stage, d, u, u0, o, ctr, st, which);
+    FieldsRW<5> wo{{Wout.rho, Wout.mx, Wout.my, Wout.mz, Wout.E}};
+    return launch_sweeps(ph, g, dtdx, stage, d, u, u0, o, wo, ctr, cache, st, which);
 }
 
 int launch_rad_sweeps(const Geom &g, const PhysConsts &pc, double dtdx, int stage, CRad4p S, const double *rho,
-                      const double *kappaR, Rad4p D, CRad4p R, CRad4p R0, Rad4p out, Counters *ctr, cudaStream_t st,
-                      int which)
+                      const double *kappaR, Rad4p D, CRad4p R, CRad4p R0, Rad4p out, Rad4p Sout, Counters *ctr,
+                      cudaStream_t st, int which)
 {
     RadPh ph;
     ph.s[0] = S.E; ph.s[1] = S.Fx; ph.s[2] = S.Fy; ph.s[3] = S.Fz;
@@ -228,7 +281,8 @@ int launch_rad_sweeps(const Geom &g, const PhysConsts &pc, double dtdx, int stag
     ph.c = pc.c; ph.c_hat = pc.c_hat; ph.dx = pc.dx; ph.tau_corr = (pc.flags & QK_FLAG_TAU_CORR) ? 1 : 0;
     FieldsRW<4> d{{D.E, D.Fx, D.Fy, D.Fz}}, o{{out.E, out.Fx, out.Fy, out.Fz}};
     FieldsRO<4> u{{R.E, R.Fx, R.Fy, R.Fz}}, u0{{R0.E, R0.Fx, R0.Fy, R0.Fz}};
-    return launch_sweeps(ph, g, dtdx, stage, d, u, u0, o, ctr, st, which);
+    FieldsRW<4> so{{Sout.E, Sout.Fx, Sout.Fy, Sout.Fz}};
+    return launch_sweeps(ph, g, dtdx, stage, d, u, u0, o, so, ctr, nullptr, st, which);
 }
 
 }  // namespace qk

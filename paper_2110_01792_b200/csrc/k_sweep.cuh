@@ -145,9 +145,11 @@ __global__ void __launch_bounds__(32 * SW_XROWS, QK_SW_XMINB) sweep_x_kernel(PH 
 template <class PH, int DIR, int MODE>
 __global__ void __launch_bounds__(SW_NT, MODE == 2 ? QK_SW_MINB2 : QK_SW_MINB1) sweep_march_kernel(PH ph, Geom g, int len, FieldsRW<PH::NV> D, RkArgs rk,
                                                             FieldsRO<PH::NV> U, FieldsRO<PH::NV> U0,
-                                                            FieldsRW<PH::NV> out, Counters *ctr)
+                                                            FieldsRW<PH::NV> out, FieldsRW<PH::NV> pout, Counters *ctr,
+                                                            StateCache *cache)
 {
     constexpr int NV = PH::NV;
+    typename PH::Tail tail;                             // per-thread reduction state of the MODE 2 epilogue
     __shared__ double ring[5 * SW_NR * SW_NT];          // [slot][var][thread], thread-private columns
     const int tid = threadIdx.x;
     const int i = blockIdx.x * SW_NT + tid;
@@ -219,6 +221,7 @@ __global__ void __launch_bounds__(SW_NT, MODE == 2 ? QK_SW_MINB2 : QK_SW_MINB1) 
             if (PH::COUNTS && active && ((mm >= m0 && mm < m1) || mm == n_m)) nguard += gd;
         }
         if (m >= m0 && active) {
+            double fresh[NV];
 #pragma unroll
             for (int v = 0; v < NV; ++v) {
                 const double div = din[v] + (Fhi[v] - Flo[v]);
@@ -226,15 +229,19 @@ __global__ void __launch_bounds__(SW_NT, MODE == 2 ? QK_SW_MINB2 : QK_SW_MINB1) 
                     D.f[v][cidx] = div;
                 } else {
                     const double us = u[v] - rk.dtdx * div;
-                    out.f[v][cidx] = rk.stage == 0 ? us : 0.5 * u0[v] + 0.5 * us;
+                    fresh[v] = rk.stage == 0 ? us : 0.5 * u0[v] + 0.5 * us;
+                    out.f[v][cidx] = fresh[v];
                 }
             }
+            // the reconstruction variables of the updated cell, for the next stage (and its CFL speed)
+            if (MODE == 2) ph.finish(cidx, fresh, pout, rk.stage == 1, tail);
         }
 #pragma unroll
         for (int v = 0; v < NV; ++v) { hiP[v] = hi[v]; Flo[v] = Fhi[v]; }
         const int t = r0; r0 = r1; r1 = r2; r2 = r3; r3 = r4; r4 = t;
     }
     if (PH::COUNTS) sweep_count(ctr, nfall, nguard);
+    if (MODE == 2) ph.finish_block(tail, rk.stage == 1, ctr, cache);
 }
 
 }  // namespace qk

@@ -18,7 +18,10 @@ using namespace qk;
 namespace {
 
 constexpr int N_STAGE = 5;          // U^(1) (hydro) / first 4 reused for radiation
-constexpr int N_SCRATCH_REF = 5 + 15;  // unfused path: primitives + 3 x 5 flux fields
+constexpr int N_SCRATCH_REF = 28;   // unfused path: primitives + 3 x 5 flux fields (0..19); sweep path: see SC_*
+// scratch fields of the sweep path: two primitive sets W (ping-pong between RK stages), the flux-difference
+// accumulators D, the three directional flattening coefficients, two radiation sets S = (E_r, f)
+constexpr int SC_WA = 0, SC_D = 5, SC_CHI3 = 10, SC_WB = 15, SC_SA = 20, SC_SB = 24;
 constexpr size_t COUNTER_BYTES = 256;
 
 inline size_t field_stride(const Geom &g) { return ((size_t)g.ntot + 31) / 32 * 32; }
@@ -39,6 +42,11 @@ struct qk_ctx {
     double *chi;
     double *scratch[N_SCRATCH_REF];
     Counters *ctr;
+    StateCache *cache;
+    // sweep path: which scratch set holds the reconstruction variables of the current state (interior
+    // cells), and whether it / the cached CFL speed still describe the state
+    int w_cur, s_cur;
+    bool w_valid, s_valid, smax_valid;
     int path;              // QK_PATH_*
     long long launches;
     int last_nsub;
@@ -66,6 +74,7 @@ int carve(qk_ctx *c)
     c->chi = p; p += fs;
     for (int f = 0; f < N_SCRATCH_REF; ++f) { c->scratch[f] = p; p += fs; }
     c->ctr = (Counters *)p;
+    c->cache = (StateCache *)((char *)p + 128);
     // zero everything once so ghost cells and unused corners are defined
     if (cudaMemsetAsync(c->base, 0, c->bytes, c->stream) != cudaSuccess) return QK_ECUDA;
     c->ready = true;
@@ -187,28 +196,37 @@ void hydro_stage_fused(qk_ctx *c, double dtdx, int stage, double *const *U, doub
     }
 }
 
-void hydro_stage_sweep(qk_ctx *c, double dtdx, int stage, double *const *U, double *const *U0, double *const *out)
+// Sweep path.  W_in holds the primitives of U (interior cells when `w_ready`; otherwise they are computed
+// here for every cell from the ghost-filled U).  The z sweep writes the updated state and its primitives
+// W_out (interior), and after the last stage the CFL speed of the new state.
+void hydro_stage_sweep(qk_ctx *c, double dtdx, int stage, double *const *U, double *const *U0, double *const *out,
+                       double *const *W, double *const *Wout, bool w_ready)
 {
     const Geom &g = c->g;
-    double *const *W = &c->scratch[0];
-    double *const *D = &c->scratch[5];
-    { Scope s(c, K_PRIM); s.done(launch_prim(g, c->pc.gamma, ch5(U), h5(W), c->ctr, c->stream)); }
+    double *const *D = &c->scratch[SC_D];
+    if (w_ready) {
+        fill_fields(c, W, 5);            // periodic / outflow images commute with the pointwise cons -> prim map
+    } else {
+        fill_fields(c, U, 5);
+        Scope s(c, K_PRIM);
+        s.done(launch_prim(g, c->pc.gamma, ch5(U), h5(W), c->ctr, c->stream));
+    }
     {
         Scope s(c, K_FLATTEN);
-        s.done(launch_chi_two_pass(g, c->pc.gamma, ch5(W), c->scratch[10], c->scratch[11], c->scratch[12], c->chi,
-                                   c->stream));
+        s.done(launch_chi_two_pass(g, c->pc.gamma, ch5(W), c->scratch[SC_CHI3], c->scratch[SC_CHI3 + 1],
+                                   c->scratch[SC_CHI3 + 2], c->chi, c->stream));
     }
     for (int d = 0; d < 3; ++d) {
         Scope s(c, K_HYDRO_SWEEP_X + d);
-        s.done(launch_hydro_sweeps(g, c->pc.gamma, dtdx, stage, ch5(W), c->chi, h5(D), ch5(U), ch5(U0), h5(out), c->ctr,
-                                   c->stream, 1 << d));
+        s.done(launch_hydro_sweeps(g, c->pc.gamma, dtdx, stage, ch5(W), c->chi, h5(D), ch5(U), ch5(U0), h5(out), h5(Wout),
+                                   c->ctr, c->cache, c->stream, 1 << d));
     }
 }
 
 void hydro_stage(qk_ctx *c, double dtdx, int stage, double *const *U, double *const *U0, double *const *out)
 {
+    fill_fields(c, U, 5);
     if (c->path == QK_PATH_FUSED) hydro_stage_fused(c, dtdx, stage, U, U0, out);
-    else if (c->path == QK_PATH_SWEEP) hydro_stage_sweep(c, dtdx, stage, U, U0, out);
     else hydro_stage_unfused(c, dtdx, stage, U, U0, out);
 }
 
@@ -217,10 +235,21 @@ int do_hydro_step(qk_ctx *c, double dt)
     const double dtdx = dt / c->pc.dx;
     double *const *Un = &c->state[QK_RHO];
     double *const *U1 = &c->stage[0];
-    fill_fields(c, Un, 5);
-    hydro_stage(c, dtdx, 0, Un, Un, U1);
-    fill_fields(c, U1, 5);
-    hydro_stage(c, dtdx, 1, U1, Un, Un);
+    if (c->path == QK_PATH_SWEEP) {
+        double *const *W0 = &c->scratch[c->w_cur ? SC_WB : SC_WA];
+        double *const *W1 = &c->scratch[c->w_cur ? SC_WA : SC_WB];
+        hydro_stage_sweep(c, dtdx, 0, Un, Un, U1, W0, W1, c->w_valid);
+        cudaMemsetAsync(c->cache, 0, sizeof(StateCache), c->stream);
+        hydro_stage_sweep(c, dtdx, 1, U1, Un, Un, W1, W0, true);
+        c->w_valid = true;               // W0 = primitives of the new state, cache = its CFL speed
+        c->smax_valid = true;
+    } else {
+        hydro_stage(c, dtdx, 0, Un, Un, U1);
+        hydro_stage(c, dtdx, 1, U1, Un, Un);
+        c->w_valid = false;              // these paths use the scratch fields for their own intermediates
+        c->s_valid = false;
+        c->smax_valid = false;
+    }
     return check_launch();
 }
 
@@ -252,23 +281,32 @@ void rad_stage_fused(qk_ctx *c, double dtdx, int stage, double *const *R, double
                             c->ctr, c->stream));
 }
 
-void rad_stage_sweep(qk_ctx *c, double dtdx, int stage, double *const *R, double *const *R0, double *const *out)
+void rad_stage_sweep(qk_ctx *c, double dtdx, int stage, double *const *R, double *const *R0, double *const *out,
+                     double *const *S, double *const *Sout, bool s_ready, bool first)
 {
     const Geom &g = c->g;
-    double *const *S = &c->scratch[0];
-    double *const *D = &c->scratch[5];
-    { Scope s(c, K_RAD_PRIM); s.done(launch_rad_prim(g, c->pc.c, cr4(R), r4(S), c->ctr, c->stream)); }
+    double *const *D = &c->scratch[SC_D];
+    // rho and kappa_R ghosts feed tau_face at the domain faces (first stage of a transport step only)
+    double *list[6];
+    int n = 0;
+    double *const *src = s_ready ? S : R;
+    for (int f = 0; f < 4; ++f) list[n++] = src[f];
+    if (first) { list[n++] = c->state[QK_RHO]; list[n++] = c->state[QK_KAPPA_R]; }
+    fill_fields(c, list, n);
+    if (!s_ready) {
+        Scope s(c, K_RAD_PRIM);
+        s.done(launch_rad_prim(g, c->pc.c, cr4(R), r4(S), c->ctr, c->stream));
+    }
     for (int d = 0; d < 3; ++d) {
         Scope s(c, K_RAD_SWEEP_X + d);
         s.done(launch_rad_sweeps(g, c->pc, dtdx, stage, cr4(S), c->state[QK_RHO], c->state[QK_KAPPA_R], r4(D), cr4(R),
-                                 cr4(R0), r4(out), c->ctr, c->stream, 1 << d));
+                                 cr4(R0), r4(out), r4(Sout), c->ctr, c->stream, 1 << d));
     }
 }
 
 void rad_stage(qk_ctx *c, double dtdx, int stage, double *const *R, double *const *R0, double *const *out)
 {
     if (c->path == QK_PATH_FUSED) rad_stage_fused(c, dtdx, stage, R, R0, out);
-    else if (c->path == QK_PATH_SWEEP) rad_stage_sweep(c, dtdx, stage, R, R0, out);
     else rad_stage_unfused(c, dtdx, stage, R, R0, out);
 }
 
@@ -277,21 +315,41 @@ int do_rad_transport(qk_ctx *c, double dt)
     const double dtdx = dt / c->pc.dx;
     double *const *Rn = &c->state[QK_ER];
     double *const *R1 = &c->stage[0];
-    // rho and kappa_R ghosts feed tau_face at the domain faces
-    double *first[6] = {Rn[0], Rn[1], Rn[2], Rn[3], c->state[QK_RHO], c->state[QK_KAPPA_R]};
-    fill_fields(c, first, 6);
-    rad_stage(c, dtdx, 0, Rn, Rn, R1);
-    fill_fields(c, R1, 4);
-    rad_stage(c, dtdx, 1, R1, Rn, Rn);
+    if (c->path == QK_PATH_SWEEP) {
+        double *const *S0 = &c->scratch[c->s_cur ? SC_SB : SC_SA];
+        double *const *S1 = &c->scratch[c->s_cur ? SC_SA : SC_SB];
+        rad_stage_sweep(c, dtdx, 0, Rn, Rn, R1, S0, S1, c->s_valid, true);
+        rad_stage_sweep(c, dtdx, 1, R1, Rn, Rn, S1, S0, true, false);
+        c->s_valid = true;
+    } else {
+        double *first[6] = {Rn[0], Rn[1], Rn[2], Rn[3], c->state[QK_RHO], c->state[QK_KAPPA_R]};
+        fill_fields(c, first, 6);
+        rad_stage(c, dtdx, 0, Rn, Rn, R1);
+        fill_fields(c, R1, 4);
+        rad_stage(c, dtdx, 1, R1, Rn, Rn);
+        c->w_valid = false;
+        c->s_valid = false;
+    }
     return check_launch();
 }
 
 int do_exchange(qk_ctx *c, double dt)
 {
     double *const *s = c->state;
+    const bool sweep = c->path == QK_PATH_SWEEP;
+    Hydro5 W{nullptr, nullptr, nullptr, nullptr, nullptr};
+    Rad4p S{nullptr, nullptr, nullptr, nullptr};
+    if (sweep) {     // the exchange rewrites rho v, E, E_r, F_r: it also refreshes what the next stages read
+        W = h5(&c->scratch[c->w_cur ? SC_WB : SC_WA]);
+        S = r4(&c->scratch[c->s_cur ? SC_SB : SC_SA]);
+        cudaMemsetAsync(c->cache, 0, sizeof(StateCache), c->stream);
+    }
     Scope sc(c, K_EXCHANGE);
     sc.done(launch_exchange(c->g, c->pc, dt, s[QK_RHO], s[QK_MX], s[QK_MY], s[QK_MZ], s[QK_E], s[QK_ER], s[QK_FX],
-                            s[QK_FY], s[QK_FZ], s[QK_KAPPA_P], s[QK_KAPPA_R], c->ctr, c->stream));
+                            s[QK_FY], s[QK_FZ], s[QK_KAPPA_P], s[QK_KAPPA_R], W, S, c->ctr, c->cache, c->stream));
+    c->w_valid = sweep;
+    c->s_valid = sweep;
+    c->smax_valid = sweep;
     return check_launch();
 }
 
@@ -330,7 +388,8 @@ int qk_init(int nx, int ny, int nz, double dx, double gamma, double c_hat, doubl
     x->pc.a_rad = 1.0; x->pc.kB_mu = 1.0; x->pc.cfl = 0.3; x->pc.newton_tol = 1e-10;
     x->pc.newton_maxit = 400; x->pc.nsub_max = 10; x->pc.flags = QK_FLAG_TAU_CORR; x->pc.bc = boundary;
     x->stream = nullptr; x->device = dev; x->base = nullptr; x->bytes = 0; x->owns = false; x->ready = false;
-    x->path = QK_PATH_SWEEP; x->launches = 0; x->last_nsub = 0; x->profiling = false;
+    x->path = QK_PATH_SWEEP; x->w_cur = 0; x->s_cur = 0; x->w_valid = false; x->s_valid = false; x->smax_valid = false;
+    x->launches = 0; x->last_nsub = 0; x->profiling = false;
     *out = x;
     return QK_OK;
 }
@@ -388,6 +447,7 @@ int qk_set_path(qk_ctx *c, int path)
 {
     if (!c || path < QK_PATH_FUSED || path > QK_PATH_SWEEP) return QK_EINVAL;
     c->path = path;
+    c->w_valid = false; c->s_valid = false;
     return QK_OK;
 }
 
@@ -396,6 +456,7 @@ int qk_set_state(qk_ctx *c, int field, const double *interior)
     if (!c || field < 0 || field >= QK_NFIELDS || !interior) return QK_EINVAL;
     int rc = ensure_storage(c);
     if (rc) return rc;
+    c->w_valid = false; c->s_valid = false; c->smax_valid = false;
     rc = copy_interior(c, c->state[field], const_cast<double *>(interior), true);
     // pageable host memory may be reused by the caller as soon as we return
     if (rc == QK_OK && !is_device_ptr(interior) && cudaStreamSynchronize(c->stream) != cudaSuccess) rc = QK_ECUDA;
@@ -417,6 +478,7 @@ int qk_set_raw(qk_ctx *c, int field, const double *with_ghosts)
     if (!c || field < 0 || field >= QK_NFIELDS || !with_ghosts) return QK_EINVAL;
     int rc = ensure_storage(c);
     if (rc) return rc;
+    c->w_valid = false; c->s_valid = false; c->smax_valid = false;
     if (cudaMemcpyAsync(c->state[field], with_ghosts, (size_t)c->g.ntot * sizeof(double), cudaMemcpyDefault,
                         c->stream) != cudaSuccess) return QK_ECUDA;
     return cudaStreamSynchronize(c->stream) == cudaSuccess ? QK_OK : QK_ECUDA;
@@ -449,14 +511,14 @@ int qk_fill_boundary(qk_ctx *c, int which)
 double qk_cfl_dt(qk_ctx *c)
 {
     if (!c || ensure_storage(c) != QK_OK) return NAN;
-    // only the two CFL words are cleared: the step counters stay readable through qk_last_info
-    cudaMemsetAsync(&c->ctr->smax_bits, 0, 2 * sizeof(long long), c->stream);
-    {
+    if (!c->smax_valid) {                // otherwise the kernel that wrote the state left its speed in the cache
+        cudaMemsetAsync(c->cache, 0, sizeof(StateCache), c->stream);
         Scope s(c, K_CFL);
-        s.done(launch_cfl(c->g, c->pc.gamma, ch5(&c->state[QK_RHO]), c->ctr, c->stream));
+        s.done(launch_cfl(c->g, c->pc.gamma, ch5(&c->state[QK_RHO]), c->cache, c->stream));
+        c->smax_valid = true;
     }
     unsigned long long host[2];
-    if (cudaMemcpyAsync(host, &c->ctr->smax_bits, sizeof(host), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+    if (cudaMemcpyAsync(host, c->cache, sizeof(host), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
         cudaStreamSynchronize(c->stream) != cudaSuccess) { cudaGetLastError(); return NAN; }
     if (host[1] != 0) return NAN;
     double smax;
@@ -544,7 +606,9 @@ int qk_last_info(qk_ctx *c, qk_info *out)
     int rc = ensure_storage(c);
     if (rc) return rc;
     Counters h;
+    StateCache sc;
     if (cudaMemcpyAsync(&h, c->ctr, sizeof(h), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+        cudaMemcpyAsync(&sc, c->cache, sizeof(sc), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
         cudaStreamSynchronize(c->stream) != cudaSuccess) { cudaGetLastError(); return QK_ECUDA; }
     out->nsub = c->last_nsub;
     out->newton_max_iters = h.newton_max;
@@ -553,7 +617,8 @@ int qk_last_info(qk_ctx *c, qk_info *out)
     out->bad_state_cells = h.bad_state;
     out->fallback_states = h.fallback;
     out->guard_faces = h.guard;
-    out->status = h.newton_fail ? QK_ENEWTON : (h.bad_state ? QK_ESTATE : QK_OK);
+    const bool cfl_bad = c->smax_valid && sc.cfl_bad != 0;     // set by the last qk_cfl_dt / hydro step
+    out->status = h.newton_fail ? QK_ENEWTON : ((h.bad_state || cfl_bad) ? QK_ESTATE : QK_OK);
     return QK_OK;
 }
 

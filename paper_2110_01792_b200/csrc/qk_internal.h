@@ -44,6 +44,13 @@ struct Counters {
     int pad;
 };
 
+// Results that stay valid between public calls (never cleared by reset_counters): the CFL signal speed of
+// the current hydro state, written by the kernel that produced that state (or by the CFL kernel).
+struct StateCache {
+    unsigned long long smax_bits;      // bit pattern of max(|v|+c_s) over interior cells
+    long long cfl_bad;                 // interior cells with rho<=0 or P<=0
+};
+
 // Kernel classes for per-kernel timing (qk_kernel_times) -- one id per __global__ function family.
 enum KClass { K_FILL = 0, K_CFL, K_PRIM, K_FLATTEN, K_HYDRO_FLUX, K_HYDRO_UPDATE, K_HYDRO_STAGE,
               K_RAD_PRIM, K_RAD_FLUX, K_RAD_UPDATE, K_RAD_STAGE, K_EXCHANGE,
@@ -67,7 +74,7 @@ struct FillList { double *f[QK_NFIELDS]; int n; };
 
 // ---- launchers (each enqueues on `st`; returns the number of kernels launched) -----------------
 int launch_fill(const Geom &g, int bc, const FillList &fl, cudaStream_t st);
-int launch_cfl(const Geom &g, double gamma, CHydro5 U, Counters *ctr, cudaStream_t st);
+int launch_cfl(const Geom &g, double gamma, CHydro5 U, StateCache *cache, cudaStream_t st);
 
 int launch_prim(const Geom &g, double gamma, CHydro5 U, Hydro5 W, Counters *ctr, cudaStream_t st);
 int launch_flatten(const Geom &g, double gamma, CHydro5 W, double *chi, cudaStream_t st);
@@ -85,12 +92,13 @@ int launch_rad_stage(const Geom &g, const PhysConsts &pc, double dtdx, int stage
 
 // sweep path (k_sweep.cu); `which` bit 0 = x sweep, bit 1 = y sweep, bit 2 = z sweep + RK update
 int launch_hydro_sweeps(const Geom &g, double gamma, double dtdx, int stage, CHydro5 W, const double *chi, Hydro5 D,
-                        CHydro5 U, CHydro5 U0, Hydro5 out, Counters *ctr, cudaStream_t st, int which);
+                        CHydro5 U, CHydro5 U0, Hydro5 out, Hydro5 Wout, Counters *ctr, StateCache *cache, cudaStream_t st,
+                        int which);
 int launch_chi_two_pass(const Geom &g, double gamma, CHydro5 W, double *cx, double *cy, double *cz, double *chi,
                         cudaStream_t st);
 int launch_rad_sweeps(const Geom &g, const PhysConsts &pc, double dtdx, int stage, CRad4p S, const double *rho,
-                      const double *kappaR, Rad4p D, CRad4p R, CRad4p R0, Rad4p out, Counters *ctr, cudaStream_t st,
-                      int which);
+                      const double *kappaR, Rad4p D, CRad4p R, CRad4p R0, Rad4p out, Rad4p Sout, Counters *ctr,
+                      cudaStream_t st, int which);
 
 int launch_rad_prim(const Geom &g, double c, CRad4p R, Rad4p S, Counters *ctr, cudaStream_t st);
 int launch_rad_flux(const Geom &g, const PhysConsts &pc, int dir, CRad4p S, const double *rho, const double *kappaR,
@@ -100,6 +108,8 @@ int launch_rad_update(const Geom &g, double dtdx, int stage, CRad4p R, CRad4p R0
 
 int launch_exchange(const Geom &g, const PhysConsts &pc, double dt, const double *rho, double *mx, double *my,
                     double *mz, double *E, double *Er, double *Fx, double *Fy, double *Fz, const double *kP,
-                    const double *kR, Counters *ctr, cudaStream_t st);
+                    const double *kR, Hydro5 Wout, Rad4p Sout, Counters *ctr, StateCache *cache, cudaStream_t st);
+// Wout.rho == nullptr: exchange only; otherwise the kernel also writes the primitives W and the radiation
+// variables S = (E_r, f) of the updated cells and leaves the CFL speed of the new state in `cache`
 
 }  // namespace qk
