@@ -36,11 +36,16 @@ METRIC = "hydro_cell_updates_per_s"
 UNIT = "cell-updates/s"
 # algorithmic fp64 operations per cell per RK stage (counted from the
 # formulas of section 3: one evaluation of every quantity per cell / face, typical branches)
-OPS_HYDRO_STAGE = 909.0     # prim 12 + flattening 66 + 3 x (PPM 170 + HLLC 93) + update 42
-OPS_HYDRO_SWEEP = 277.0     # one direction: PPM 170 + HLLC 93 + its share of the update 14
-OPS_RAD_STAGE = 840.0       # rad prim 8 + 3 x (PPM 112 + fallback test 14 + closure/HLL 140) + update 34
-OPS_RAD_SWEEP = 277.0       # one direction: PPM 126 + closure/HLL 140 + its share of the update 11
-BYTES_EXCHANGE = 152.0
+# SURVEY.md section 8(d) / 8(a) figures (branch-free worst-case paths, div and sqrt counted as one op each):
+OPS_HYDRO_STAGE = 1240.0    # S3 12 + S4 62 + S5 810 + S6 318 + S7 38
+OPS_HYDRO_SWEEP = 388.0     # one direction of one stage: S5 270 + S6 106 + its share of S7 12
+OPS_RAD_STAGE = 1080.0      # S8 640 + S9 402 + S10 38
+OPS_RAD_SWEEP = 357.0       # one direction: S8 214 + S9 134 + its share of S10 9
+BYTES_EXCHANGE = 224.0      # 11 reads + 8 writes (eq 26-43) + the 9 reconstruction variables it leaves for the next stage
+# dram__bytes_read.sum + dram__bytes_write.sum per launch at 256^3 from the ncu --set full capture summarised in
+# profiles/r1_kernels.md (GB); not measured live, null at any other size
+NCU_TRAFFIC_GB_256 = {"hydro_sweep_x": 1.465, "hydro_sweep_y": 2.177, "hydro_sweep_z": 3.666,
+                      "rad_sweep_x": 1.337, "rad_sweep_y": 1.912, "rad_sweep_z": 3.101, "exchange": 3.750}
 
 
 def log(*a):
@@ -272,8 +277,10 @@ def roofline_alu(kernel_ms, names, ops_per_cell_per_launch, cells, peak_ops, pea
             tot, cnt = kernel_ms[nm]
             mean_ms = tot / cnt
             achieved = ops_per_cell_per_launch * cells / (mean_ms * 1e-3) / 1e12
+            traffic = NCU_TRAFFIC_GB_256.get(nm) if cells == 256 ** 3 else None
             return {"bound": "alu", "kernel": nm, "achieved": achieved, "peak": peak_ops / 1e12,
-                    "unit": "TFLOP/s", "frac": achieved / (peak_ops / 1e12), "traffic": None,
+                    "unit": "TFLOP/s", "frac": achieved / (peak_ops / 1e12),
+                    "traffic": None if traffic is None else traffic * 1e9,
                     "launch_ms": mean_ms, "launches": cnt, "peak_source": peak_note,
                     "ops_per_cell_per_launch": ops_per_cell_per_launch}
     return None
@@ -375,7 +382,8 @@ def run_ours(args):
         if ex:
             ach = BYTES_EXCHANGE * cells / (ex[0] / ex[1] * 1e-3) / 1e9
             exroof = {"bound": "hbm", "kernel": "exchange", "achieved": ach, "peak": hbm, "unit": "GB/s",
-                      "frac": ach / hbm, "traffic": None, "launch_ms": ex[0] / ex[1], "peak_source": hbm_note}
+                      "frac": ach / hbm, "traffic": NCU_TRAFFIC_GB_256["exchange"] * 1e9 if cells == 256 ** 3 else None,
+                      "launch_ms": ex[0] / ex[1], "peak_source": hbm_note}
         line["rhd"] = {
             "metric": "rhd_cell_updates_per_s", "value": rhd["value"], "unit": UNIT, "steps": rhd["steps"],
             "ms_per_step": rhd["ms"] / rhd["steps"], "nsub": rhd["info"]["nsub"],
