@@ -182,7 +182,20 @@ def run_reference(args):
 # ---------------------------------------------------------------------------------------------
 # the CUDA path
 # ---------------------------------------------------------------------------------------------
-def time_steps(torch, ctx, kind, nsteps, barrier):
+def one_step(ctx, kind, ex):
+    """qk_cfl_dt (min over ranks when the box is decomposed) + one step of the hot path."""
+    dt = ctx.qk_cfl_dt()
+    if ex is not None:
+        dt = ex.global_dt(dt)
+    if kind == "hydro":
+        ctx.qk_hydro_step(dt)
+    else:
+        ctx.qk_rhd_step(dt)
+    if ex is not None:
+        ex.check()
+
+
+def time_steps(torch, ctx, kind, nsteps, barrier, ex=None):
     """nsteps x (qk_cfl_dt + step) bracketed by barrier + synchronize, timed with CUDA events on the
     stream the kernels are launched on.  Returns milliseconds."""
     stream = torch.cuda.current_stream()
@@ -191,18 +204,14 @@ def time_steps(torch, ctx, kind, nsteps, barrier):
     torch.cuda.synchronize()
     e0.record(stream)
     for _ in range(nsteps):
-        dt = ctx.qk_cfl_dt()
-        if kind == "hydro":
-            ctx.qk_hydro_step(dt)
-        else:
-            ctx.qk_rhd_step(dt)
+        one_step(ctx, kind, ex)
     e1.record(stream)
     torch.cuda.synchronize()
     barrier()
     return e0.elapsed_time(e1)
 
 
-def time_steps_e2e(torch, ctx, kind, nsteps, host_in, host_out, barrier):
+def time_steps_e2e(torch, ctx, kind, nsteps, host_in, host_out, barrier, ex=None):
     """Same step through the C ABI with HOST (pinned) buffers: H2D of the evolving fields, step,
     D2H of the result, every step, inside the timed region."""
     stream = torch.cuda.current_stream()
@@ -214,11 +223,7 @@ def time_steps_e2e(torch, ctx, kind, nsteps, host_in, host_out, barrier):
     for _ in range(nsteps):
         for f in range(nf):
             ctx.qk_set_state(f, host_in[f])
-        dt = ctx.qk_cfl_dt()
-        if kind == "hydro":
-            ctx.qk_hydro_step(dt)
-        else:
-            ctx.qk_rhd_step(dt)
+        one_step(ctx, kind, ex)
         for f in range(nf):
             ctx.qk_get_state(f, host_out[f])
         host_in, host_out = host_out, host_in      # next step starts from this step's result
@@ -228,7 +233,8 @@ def time_steps_e2e(torch, ctx, kind, nsteps, host_in, host_out, barrier):
     return e0.elapsed_time(e1)
 
 
-def run_workload(torch, B, I, kind, n, steps, warmup, rank, world, barrier, allmax, sampler=None, path=None):
+def run_workload(torch, B, I, kind, n, steps, warmup, rank, world, barrier, allmax, sampler=None, path=None,
+                 decompose=False):
     t0 = time.time()
     params, fields = (I.config2(n=n, seed=1002 + rank) if kind == "hydro" else I.config4(n=n, seed=1004 + rank))
     log("[rank %d] %s %d^3 inputs generated in %.1f s" % (rank, kind, n, time.time() - t0))
@@ -238,16 +244,23 @@ def run_workload(torch, B, I, kind, n, steps, warmup, rank, world, barrier, allm
     with B.from_params(params, fields) as ctx:
         if path is not None:
             ctx.qk_set_path(path)
+        ex = None
+        if decompose and world > 1:
+            # one global box of n x n x (world n) cells, rank r owns the z slab r: ghost planes cross ranks by
+            # NCCL send/recv before every stage fill, dt is the minimum over ranks
+            from paper_2110_01792_b200 import decomp as D
+            ex = D.SlabExchange(ctx, rank, world, True, D.TorchTransport())
+        out["parallelism"] = ("z-slab decomposition of one %dx%dx%d box, halo exchange per RK stage (NCCL p2p), "
+                              "global min dt" % (n, n, n * world)) if ex else "1 box per GPU"
         for _ in range(warmup):
-            dt = ctx.qk_cfl_dt()
-            ctx.qk_hydro_step(dt) if kind == "hydro" else ctx.qk_rhd_step(dt)
+            one_step(ctx, kind, ex)
         ctx.set_all(fields)                        # timed steps are steps 1..K of the config
         torch.cuda.synchronize()
         l0 = ctx.qk_launch_count()
         ctx.qk_set_profiling(True)
         if sampler:
             sampler.start()
-        ms = time_steps(torch, ctx, kind, steps, barrier)
+        ms = time_steps(torch, ctx, kind, steps, barrier, ex)
         clocks = sampler.stop() if sampler else None
         ktimes = ctx.qk_kernel_times()
         ctx.qk_set_profiling(False)
@@ -260,11 +273,14 @@ def run_workload(torch, B, I, kind, n, steps, warmup, rank, world, barrier, allm
         host_a = [torch.from_numpy(np.ascontiguousarray(fields[I.FIELDS[f]])).pin_memory() for f in range(nf)]
         host_b = [torch.empty_like(t).pin_memory() for t in host_a]
         e2e_steps = max(1, min(steps, 5))
-        time_steps_e2e(torch, ctx, kind, 1, [t.clone().pin_memory() for t in host_a], host_b, barrier)  # warm
-        ms_e = allmax(time_steps_e2e(torch, ctx, kind, e2e_steps, host_a, host_b, barrier))
+        time_steps_e2e(torch, ctx, kind, 1, [t.clone().pin_memory() for t in host_a], host_b, barrier, ex)  # warm
+        ms_e = allmax(time_steps_e2e(torch, ctx, kind, e2e_steps, host_a, host_b, barrier, ex))
         out["e2e"] = {"value": world * cells * e2e_steps / (ms_e * 1e-3), "unit": UNIT,
                       "h2d_bytes_per_step": nf * cells * 8, "d2h_bytes_per_step": nf * cells * 8,
                       "ms_per_step": ms_e / e2e_steps, "steps": e2e_steps}
+        if ex is not None:
+            out["halo"] = {"exchanges": ex.calls, "bytes_sent_per_rank": ex.bytes_sent}
+            ex.detach()
     return out
 
 
@@ -331,12 +347,13 @@ def run_ours(args):
     path = {"fused": B.QK_PATH_FUSED, "unfused": B.QK_PATH_UNFUSED, "sweep": B.QK_PATH_SWEEP}[args.path]
     hyd = None
     if not args.no_hydro:
-        hyd = run_workload(torch, B, I, "hydro", n, args.steps, args.warmup, rank, world, barrier, allmax, sampler, path)
+        hyd = run_workload(torch, B, I, "hydro", n, args.steps, args.warmup, rank, world, barrier, allmax, sampler, path,
+                           decompose=not args.replicas)
     rhd = None
     if not args.no_rhd or hyd is None:
         rhd_steps = max(1, min(args.steps, args.rhd_steps))
         rhd = run_workload(torch, B, I, "rhd", n, rhd_steps, min(args.warmup, 3), rank, world, barrier, allmax,
-                           sampler if hyd is None else None, path)
+                           sampler if hyd is None else None, path, decompose=not args.replicas)
         rhd["steps"] = rhd_steps
 
     if rank != 0:
@@ -366,13 +383,15 @@ def run_ours(args):
         "config": {"workload": "BASELINE.json configs[1]: pure hydro %d^3, periodic, gamma=5/3, log-normal density, "
                                "k^-2 velocity field at rms Mach 2, CFL 0.3, qk_cfl_dt + qk_hydro_step per step" % n,
                    "cells": cells, "l2": "inputs larger than L2 (5 x %.0f MB per stage)" % (cells * 8 / 1e6),
-                   "parallelism": "1 box per GPU, no halo exchange (replicas)" if world > 1 else "1 box on 1 GPU"},
+                   "parallelism": hyd.get("parallelism", "1 box on 1 GPU") if world > 1 else "1 box on 1 GPU"},
         "e2e": hyd["e2e"], "gpu_launches": hyd["launches"], "clocks": hyd["clocks"],
         "roofline": roof,
         "kernel_ms": {k: {"total_ms": v[0], "groups": v[1]} for k, v in hyd["kernel_ms"].items()},
         "peaks": {"fp64_dmul_dadd_lane_ops_per_s": peak_ops, "fp64_dfma_lane_ops_per_s": peak_fma,
                   "hbm_gbs": hbm, "hbm_source": hbm_note},
     }
+    if hyd.get("halo"):
+        line["halo"] = hyd["halo"]
     if rhd is not None:
         ex = rhd["kernel_ms"].get("exchange")
         names, ops = family(rhd["kernel_ms"], "rad_stage", ["rad_sweep_x", "rad_sweep_y", "rad_sweep_z", "rad_flux"],
@@ -419,6 +438,8 @@ def main():
     ap.add_argument("--rhd-steps", type=int, default=10)
     ap.add_argument("--ref-size", type=int, default=128, help="edge of the oracle's bounded sample")
     ap.add_argument("--path", default="sweep", choices=["fused", "unfused", "sweep"], help="stage kernel family")
+    ap.add_argument("--replicas", action="store_true",
+                    help="N>1: independent boxes per GPU instead of one z-slab-decomposed global box")
     ap.add_argument("--no-rhd", action="store_true")
     ap.add_argument("--no-hydro", action="store_true", help="profiling aid: run only the RHD workload")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -48,6 +48,11 @@ enum { QK_FLAG_TAU_CORR = 1,        /* guarded optical-depth correction of the E
 
 enum { QK_FILL_HYDRO = 1, QK_FILL_RAD = 2, QK_FILL_OPACITY = 4, QK_FILL_ALL = 7 };
 
+/* z-slab domain decomposition (one box per GPU; the paper's pattern: one ghost exchange per
+ * RK stage).  Faces named here border another rank's slab. */
+enum { QK_FACE_ZLO = 1, QK_FACE_ZHI = 2 };
+typedef void (*qk_halo_fn)(void *user, int nfields);
+
 /* Counters of the most recent step call (qk_hydro_step / qk_rad_step / qk_rhd_step / qk_exchange
  * / qk_rad_transport), summed over the substeps of a qk_rhd_step. */
 typedef struct qk_info {
@@ -107,6 +112,21 @@ int qk_get_raw(qk_ctx *ctx, int field, double *with_ghosts);
  * every ghost cell <- the interior cell its three indices map to, periodic wrap or
  * nearest-interior copy ("B.C. fill"). */
 int qk_fill_boundary(qk_ctx *ctx, int which);
+
+/* Declare the z faces in `faces` (QK_FACE_* bits) as inter-rank faces.  Before every ghost fill the library then
+ * calls fn(user, nfields) on the calling thread; inside it the caller moves the halos of the nfields fields about
+ * to be filled: qk_halo_pack(face, buf) copies the QK_NG interior planes next to `face` of each of them into the
+ * DEVICE buffer buf (nfields * qk_halo_doubles() doubles, field-major, planes ascending in z, ny*nx interior cells
+ * per plane), the caller sends it to the neighbour (NCCL send/recv, peer copy, ...), and qk_halo_unpack(face, buf)
+ * writes a received buffer into the QK_NG ghost planes beyond `face`.  All on the context's stream.  After fn
+ * returns the library fills the remaining ghost cells (x, y images and the physical z faces).  The result equals
+ * the single-box update bit for bit.  faces = 0 or fn = NULL switches the decomposition off.  Needs nz >= QK_NG.
+ * qk_halo_pack / qk_halo_unpack return QK_EINVAL outside the callback.  qk_cfl_dt stays local: the caller takes
+ * the minimum over ranks. */
+int qk_set_halo_exchange(qk_ctx *ctx, unsigned faces, qk_halo_fn fn, void *user);
+size_t qk_halo_doubles(const qk_ctx *ctx);          /* QK_NG * ny * nx: doubles per field per face */
+int qk_halo_pack(qk_ctx *ctx, int face, double *dev_buf);
+int qk_halo_unpack(qk_ctx *ctx, int face, const double *dev_buf);
 
 /* eq 21: dt = CFL dx / max_cells(|v| + c_s), |v| the vector magnitude,
  * further limited to nsub_max CFL dx / c_hat when c_hat > 0.  Synchronises.

@@ -28,7 +28,7 @@ EXPORTS = [
     "qk_cfl_dt", "qk_hydro_step", "qk_rad_transport", "qk_exchange", "qk_rad_step", "qk_rhd_step",
     "qk_nsub_for", "qk_last_info", "qk_launch_count", "qk_set_path", "qk_set_profiling",
     "qk_kernel_class_count", "qk_kernel_class_name", "qk_kernel_times", "qk_version", "qk_fp64_probe",
-    "qk_selftest_divsqrt",
+    "qk_selftest_divsqrt", "qk_set_halo_exchange", "qk_halo_doubles", "qk_halo_pack", "qk_halo_unpack",
 ]
 
 
@@ -36,6 +36,10 @@ class qk_info(C.Structure):
     _fields_ = [("nsub", C.c_int), ("newton_max_iters", C.c_int), ("newton_fail_cells", C.c_longlong),
                 ("newton_total_iters", C.c_longlong), ("bad_state_cells", C.c_longlong),
                 ("fallback_states", C.c_longlong), ("guard_faces", C.c_longlong), ("status", C.c_int)]
+
+
+QK_FACE_ZLO, QK_FACE_ZHI = 1, 2
+HALO_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_int)
 
 
 class QkError(RuntimeError):
@@ -85,6 +89,10 @@ def lib():
         "qk_version": (C.c_char_p, []),
         "qk_fp64_probe": (i, [i, i, p, C.POINTER(d)]),
         "qk_selftest_divsqrt": (i, [ll, C.c_ulonglong, i, p, C.POINTER(ll)]),
+        "qk_set_halo_exchange": (i, [p, u, HALO_FN, p]),
+        "qk_halo_doubles": (C.c_size_t, [p]),
+        "qk_halo_pack": (i, [p, i, p]),
+        "qk_halo_unpack": (i, [p, i, p]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)
@@ -202,6 +210,29 @@ class Context:
             out = np.empty((self.nz + 2 * NG, self.ny + 2 * NG, self.nx + 2 * NG), dtype=np.float64)
         _check(self.L.qk_get_raw(self.h, field, _ptr(out)), "qk_get_raw")
         return out
+
+    def qk_set_halo_exchange(self, faces, fn):
+        """fn(nfields) is called before every ghost fill (see include/qk.h); None switches it off."""
+        if fn is None or not faces:
+            self._halo_cb = None
+            _check(self.L.qk_set_halo_exchange(self.h, 0, C.cast(None, HALO_FN), None), "qk_set_halo_exchange")
+            return
+        self._halo_cb = HALO_FN(lambda user, nfields: fn(nfields))     # keep the thunk alive
+        _check(self.L.qk_set_halo_exchange(self.h, faces, self._halo_cb, None), "qk_set_halo_exchange")
+
+    def new_buffer(self, ndoubles):
+        """Device buffer for halo planes (PyTorch owns the memory)."""
+        import torch
+        return torch.empty(ndoubles, dtype=torch.float64, device=self.device)
+
+    def qk_halo_doubles(self):
+        return int(self.L.qk_halo_doubles(self.h))
+
+    def qk_halo_pack(self, face, buf):
+        _check(self.L.qk_halo_pack(self.h, face, _ptr(buf)), "qk_halo_pack")
+
+    def qk_halo_unpack(self, face, buf):
+        _check(self.L.qk_halo_unpack(self.h, face, _ptr(buf)), "qk_halo_unpack")
 
     def qk_fill_boundary(self, which=QK_FILL_ALL):
         _check(self.L.qk_fill_boundary(self.h, which), "qk_fill_boundary")

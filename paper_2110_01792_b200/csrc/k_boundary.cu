@@ -23,7 +23,9 @@ __device__ __forceinline__ int wrap_index(int i, int n, int bc)
     return i < 0 ? 0 : n - 1;
 }
 
-__global__ void __launch_bounds__(256) fill_ghost_kernel(Geom g, int bc, FillList fl)
+// `ext` = QK_FACE_* bits of the z faces that border another rank's slab: their ghost planes already hold the
+// neighbour's cells at the interior (i, j) positions (qk_halo_unpack), so only their x / y images are filled.
+__global__ void __launch_bounds__(256) fill_ghost_kernel(Geom g, int bc, unsigned ext, FillList fl)
 {
     const long long nZ = 2LL * NG * g.py * g.px;
     const long long nY = 2LL * NG * g.nz * g.px;
@@ -53,21 +55,56 @@ __global__ void __launch_bounds__(256) fill_ghost_kernel(Geom g, int bc, FillLis
             j = row - k * g.ny;
             i = ii < NG ? ii - NG : g.nx + (ii - NG);
         }
+        const bool k_ext = (k < 0 && (ext & QK_FACE_ZLO)) || (k >= g.nz && (ext & QK_FACE_ZHI));
         const int dst = g.at(i, j, k);
-        const int src = g.at(wrap_index(i, g.nx, bc), wrap_index(j, g.ny, bc), wrap_index(k, g.nz, bc));
+        const int src = g.at(wrap_index(i, g.nx, bc), wrap_index(j, g.ny, bc), k_ext ? k : wrap_index(k, g.nz, bc));
+        if (src == dst) continue;
 #pragma unroll 1
         for (int f = 0; f < fl.n; ++f) fl.f[f][dst] = fl.f[f][src];
     }
 }
 
-int launch_fill(const Geom &g, int bc, const FillList &fl, cudaStream_t st)
+// Halo planes of a z face: NG planes x ny x nx interior cells per field, field-major, planes ascending in k.
+// pack: the NG interior planes next to the face -> buf;  unpack: buf -> the NG ghost planes beyond the face.
+__global__ void __launch_bounds__(256) halo_copy_kernel(Geom g, int face_hi, int unpack, FillList fl, double *buf)
+{
+    const long long per_field = (long long)NG * g.ny * g.nx;
+    const long long total = per_field * fl.n;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < total;
+         t += (long long)gridDim.x * blockDim.x) {
+        const int f = (int)(t / per_field);
+        const long long u = t - (long long)f * per_field;
+        const int row = (int)(u / g.nx);
+        const int i = (int)(u - (long long)row * g.nx);
+        const int kk = row / g.ny;
+        const int j = row - kk * g.ny;
+        int k;
+        if (unpack) k = face_hi ? g.nz + kk : kk - NG;
+        else        k = face_hi ? g.nz - NG + kk : kk;
+        const int cidx = g.at(i, j, k);
+        if (unpack) fl.f[f][cidx] = buf[t];
+        else        buf[t] = fl.f[f][cidx];
+    }
+}
+
+int launch_halo_copy(const Geom &g, int face_hi, int unpack, const FillList &fl, double *buf, cudaStream_t st)
+{
+    if (fl.n <= 0) return 0;
+    const long long total = (long long)NG * g.ny * g.nx * fl.n;
+    long long blocks = (total + 255) / 256;
+    if (blocks > 148LL * 16) blocks = 148LL * 16;
+    halo_copy_kernel<<<(unsigned)blocks, 256, 0, st>>>(g, face_hi, unpack, fl, buf);
+    return 1;
+}
+
+int launch_fill(const Geom &g, int bc, unsigned ext, const FillList &fl, cudaStream_t st)
 {
     if (fl.n <= 0) return 0;
     const long long total = 2LL * NG * ((long long)g.py * g.px + (long long)g.nz * g.px + (long long)g.nz * g.ny);
     long long blocks = (total + 255) / 256;
     const long long cap = 148LL * 32;
     if (blocks > cap) blocks = cap;
-    fill_ghost_kernel<<<(unsigned)blocks, 256, 0, st>>>(g, bc, fl);
+    fill_ghost_kernel<<<(unsigned)blocks, 256, 0, st>>>(g, bc, ext, fl);
     return 1;
 }
 

@@ -48,6 +48,12 @@ struct qk_ctx {
     int w_cur, s_cur;
     bool w_valid, s_valid, smax_valid;
     int path;              // QK_PATH_*
+    // z-slab decomposition: inter-rank faces, the caller's halo mover, and the field list of the fill in progress
+    unsigned ext_faces;
+    qk_halo_fn halo_fn;
+    void *halo_user;
+    FillList pending;
+    bool in_halo_cb;
     long long launches;
     int last_nsub;
     // per-kernel-class event timing
@@ -160,7 +166,13 @@ void fill_fields(qk_ctx *c, double *const *fields, int n)
     fl.n = n;
     for (int i = 0; i < n; ++i) fl.f[i] = fields[i];
     Scope s(c, K_FILL);
-    s.done(launch_fill(c->g, c->pc.bc, fl, c->stream));
+    if (c->ext_faces && c->halo_fn) {      // neighbours' planes first, then the x / y images of everything
+        c->pending = fl;
+        c->in_halo_cb = true;
+        c->halo_fn(c->halo_user, n);
+        c->in_halo_cb = false;
+    }
+    s.done(launch_fill(c->g, c->pc.bc, c->ext_faces, fl, c->stream));
 }
 
 // ---- hydro: SSP-RK2 ------------------------------------------------------------------
@@ -389,6 +401,7 @@ int qk_init(int nx, int ny, int nz, double dx, double gamma, double c_hat, doubl
     x->pc.newton_maxit = 400; x->pc.nsub_max = 10; x->pc.flags = QK_FLAG_TAU_CORR; x->pc.bc = boundary;
     x->stream = nullptr; x->device = dev; x->base = nullptr; x->bytes = 0; x->owns = false; x->ready = false;
     x->path = QK_PATH_SWEEP; x->w_cur = 0; x->s_cur = 0; x->w_valid = false; x->s_valid = false; x->smax_valid = false;
+    x->ext_faces = 0; x->halo_fn = nullptr; x->halo_user = nullptr; x->pending.n = 0; x->in_halo_cb = false;
     x->launches = 0; x->last_nsub = 0; x->profiling = false;
     *out = x;
     return QK_OK;
@@ -507,6 +520,29 @@ int qk_fill_boundary(qk_ctx *c, int which)
     fill_fields(c, list, n);
     return check_launch();
 }
+
+int qk_set_halo_exchange(qk_ctx *c, unsigned faces, qk_halo_fn fn, void *user)
+{
+    if (!c || (faces & ~(unsigned)(QK_FACE_ZLO | QK_FACE_ZHI))) return QK_EINVAL;
+    if (faces && fn && c->g.nz < NG) return QK_EINVAL;
+    c->ext_faces = fn ? faces : 0u;
+    c->halo_fn = faces ? fn : nullptr;
+    c->halo_user = user;
+    return QK_OK;
+}
+
+size_t qk_halo_doubles(const qk_ctx *c) { return c ? (size_t)NG * c->g.ny * c->g.nx : 0; }
+
+static int halo_copy(qk_ctx *c, int face, double *buf, int unpack)
+{
+    if (!c || !buf || !c->in_halo_cb || (face != QK_FACE_ZLO && face != QK_FACE_ZHI) || !(c->ext_faces & face))
+        return QK_EINVAL;
+    c->launches += launch_halo_copy(c->g, face == QK_FACE_ZHI, unpack, c->pending, buf, c->stream);
+    return check_launch();
+}
+
+int qk_halo_pack(qk_ctx *c, int face, double *dev_buf) { return halo_copy(c, face, dev_buf, 0); }
+int qk_halo_unpack(qk_ctx *c, int face, const double *dev_buf) { return halo_copy(c, face, const_cast<double *>(dev_buf), 1); }
 
 double qk_cfl_dt(qk_ctx *c)
 {

@@ -1,0 +1,122 @@
+"""z-slab domain decomposition of one global box over the ranks of a torch.distributed job
+(the paper's pattern: one ghost exchange per RK stage plus a min-reduction of the
+timestep).
+
+Host-side plumbing only: which faces border a neighbour, who the neighbours are, the order of the
+sends and receives, the reduction of dt.  The halo planes themselves are packed / unpacked by
+kernels of the library (qk_halo_pack / qk_halo_unpack) and moved by torch.distributed point-to-point
+operations (NCCL over NVLink on GPUs, gloo on CPU in the tests).  `SlabExchange` works with any
+object that has qk_set_halo_exchange / qk_halo_doubles / qk_halo_pack / qk_halo_unpack and a
+`new_buffer(ndoubles)` method, so the CPU tests drive it with a numpy stand-in.
+"""
+from __future__ import annotations
+
+FACE_ZLO, FACE_ZHI = 1, 2
+
+
+def slab_extent(nz_global: int, rank: int, world: int):
+    """(first plane, number of planes) of rank's slab: planes are dealt out as evenly as possible,
+    the first nz_global % world ranks get one more."""
+    base, extra = divmod(nz_global, world)
+    n = base + (1 if rank < extra else 0)
+    k0 = rank * base + min(rank, extra)
+    return k0, n
+
+
+def neighbours(rank: int, world: int, periodic: bool):
+    """(lower neighbour, upper neighbour) along z, None at a physical boundary."""
+    if world == 1:
+        return None, None
+    lo = rank - 1 if rank > 0 else (world - 1 if periodic else None)
+    hi = rank + 1 if rank < world - 1 else (0 if periodic else None)
+    return lo, hi
+
+
+class TorchTransport:
+    """Moves (send_lo, send_hi) to the neighbours and fills (recv_lo, recv_hi) with torch.distributed
+    point-to-point operations.  With two ranks and periodic boundaries both neighbours are the same
+    peer: messages between one pair of ranks match in posting order, so the sends are posted high
+    face first and the receives low face first (my low ghost planes are the peer's high planes)."""
+
+    def __init__(self, group=None):
+        import torch.distributed as dist
+        self.dist = dist
+        self.group = group
+
+    def exchange(self, lo, hi, send_lo, send_hi, recv_lo, recv_hi):
+        dist = self.dist
+        ops = []
+        if hi is not None:
+            ops.append(dist.P2POp(dist.isend, send_hi, hi, self.group))
+        if lo is not None:
+            ops.append(dist.P2POp(dist.isend, send_lo, lo, self.group))
+        if lo is not None:
+            ops.append(dist.P2POp(dist.irecv, recv_lo, lo, self.group))
+        if hi is not None:
+            ops.append(dist.P2POp(dist.irecv, recv_hi, hi, self.group))
+        if ops:
+            for req in dist.batch_isend_irecv(ops):
+                req.wait()
+
+    def min_over_ranks(self, x: float) -> float:
+        import torch
+        dist = self.dist
+        dev = "cuda" if dist.get_backend(self.group) == "nccl" else "cpu"
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MIN, group=self.group)
+        return float(t.item())
+
+
+class SlabExchange:
+    """Attaches the halo exchange of one rank's slab to a context."""
+
+    def __init__(self, ctx, rank: int, world: int, periodic: bool, transport):
+        self.ctx, self.transport = ctx, transport
+        self.lo, self.hi = neighbours(rank, world, periodic)
+        self.faces = (FACE_ZLO if self.lo is not None else 0) | (FACE_ZHI if self.hi is not None else 0)
+        self.per_field = ctx.qk_halo_doubles()
+        self.buffers = {}
+        self.calls = 0
+        self.bytes_sent = 0
+        self.error = None
+        ctx.qk_set_halo_exchange(self.faces, self._on_fill if self.faces else None)
+
+    def _bufs(self, nfields):
+        if nfields not in self.buffers:
+            n = nfields * self.per_field
+            self.buffers[nfields] = tuple(self.ctx.new_buffer(n) for _ in range(4))
+        return self.buffers[nfields]
+
+    def _on_fill(self, nfields):
+        # called by the library before every ghost fill; exceptions cannot cross the C frame
+        try:
+            send_lo, send_hi, recv_lo, recv_hi = self._bufs(nfields)
+            if self.lo is not None:
+                self.ctx.qk_halo_pack(FACE_ZLO, send_lo)
+            if self.hi is not None:
+                self.ctx.qk_halo_pack(FACE_ZHI, send_hi)
+            self.transport.exchange(self.lo, self.hi, send_lo, send_hi, recv_lo, recv_hi)
+            if self.lo is not None:
+                self.ctx.qk_halo_unpack(FACE_ZLO, recv_lo)
+            if self.hi is not None:
+                self.ctx.qk_halo_unpack(FACE_ZHI, recv_hi)
+            self.calls += 1
+            self.bytes_sent += 8 * nfields * self.per_field * ((self.lo is not None) + (self.hi is not None))
+        except BaseException as e:      # noqa: BLE001 -- re-raised by check() on the Python side
+            if self.error is None:
+                self.error = e
+
+    def check(self):
+        if self.error is not None:
+            e, self.error = self.error, None
+            raise e
+
+    def global_dt(self, local_dt: float) -> float:
+        """eq 21 over the whole box: the minimum of the ranks' local timesteps (NaN propagates)."""
+        if local_dt != local_dt:
+            local_dt = float("-inf")
+        dt = self.transport.min_over_ranks(local_dt)
+        return float("nan") if dt == float("-inf") else dt
+
+    def detach(self):
+        self.ctx.qk_set_halo_exchange(0, None)

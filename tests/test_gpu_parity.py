@@ -350,3 +350,87 @@ def test_rhd_config4_full_size_sampled():
     params, fields = I.config4()
     _sampled_full_size(params, fields, lambda c, dt: c.qk_rhd_step(dt), lambda g, dt: g.rhd_step(dt),
                        I.FIELDS[:9], P.TOL_ONE_STEP, halo=14, core=4, nsamples=3)
+
+
+# ------------------------------------------------------------------------------------------------
+# 8(e): z-slab decomposition -- two slabs (two contexts, two host threads, one GPU) against one box
+# ------------------------------------------------------------------------------------------------
+class _ThreadTransport:
+    """In-process stand-in for the NCCL transport of decomp.TorchTransport: the two slabs live on the same
+    GPU and stream, halo buffers change hands through queues between the two driving threads."""
+
+    def __init__(self, rank, world, queues, barrier, shared):
+        self.rank, self.world, self.q, self.barrier, self.shared = rank, world, queues, barrier, shared
+
+    def exchange(self, lo, hi, send_lo, send_hi, recv_lo, recv_hi):
+        if hi is not None:
+            self.q[(self.rank, hi, "up")].put(send_hi.clone())
+        if lo is not None:
+            self.q[(self.rank, lo, "down")].put(send_lo.clone())
+        if lo is not None:
+            recv_lo.copy_(self.q[(lo, self.rank, "up")].get(timeout=60))
+        if hi is not None:
+            recv_hi.copy_(self.q[(hi, self.rank, "down")].get(timeout=60))
+
+    def min_over_ranks(self, x):
+        self.shared[self.rank] = x
+        self.barrier.wait(timeout=60)
+        m = min(self.shared)
+        self.barrier.wait(timeout=60)
+        return m
+
+
+def _run_decomposed(params, fields, world, nsteps, kind):
+    import queue
+    import threading
+    from paper_2110_01792_b200 import decomp as D
+    nzg = params["nz"]
+    periodic = params["bc"] == I.BC_PERIODIC
+    queues = {(a, b, d): queue.Queue() for a in range(world) for b in range(world) for d in ("up", "down")}
+    barrier, shared = threading.Barrier(world), [0.0] * world
+    results, errors = [None] * world, []
+
+    def drive(rank):
+        try:
+            import torch
+            torch.cuda.set_device(0)
+            k0, nz = D.slab_extent(nzg, rank, world)
+            p = dict(params, nz=nz)
+            f = {n: np.ascontiguousarray(a[k0:k0 + nz]) for n, a in fields.items()}
+            with P.make_gpu(p, f) as ctx:
+                ex = D.SlabExchange(ctx, rank, world, periodic, _ThreadTransport(rank, world, queues, barrier, shared))
+                for _ in range(nsteps):
+                    dt = ex.global_dt(ctx.qk_cfl_dt())
+                    ctx.qk_hydro_step(dt) if kind == "hydro" else ctx.qk_rhd_step(dt)
+                    ex.check()
+                results[rank] = (ctx.get_all(I.FIELDS[:9]), ctx.qk_last_info(), ex.calls)
+        except BaseException as e:  # noqa: BLE001
+            errors.append((rank, repr(e)))
+            barrier.abort()
+
+    threads = [threading.Thread(target=drive, args=(r,)) for r in range(world)]
+    [t.start() for t in threads]
+    [t.join(timeout=300) for t in threads]
+    assert not errors, errors
+    return results
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("bc", [I.BC_PERIODIC, I.BC_OUTFLOW], ids=["periodic", "outflow"])
+@pytest.mark.parametrize("kind,world", [("hydro", 2), ("hydro", 3), ("rhd", 2)])
+def test_slab_decomposition_is_bitwise_the_single_box(kind, world, bc):
+    params, fields = (I.ragged_hydro(bc=bc) if kind == "hydro" else I.ragged_rhd(bc=bc))
+    nsteps = 3 if kind == "hydro" else 2
+    with P.make_gpu(params, fields) as ctx:
+        for _ in range(nsteps):
+            dt = ctx.qk_cfl_dt()
+            ctx.qk_hydro_step(dt) if kind == "hydro" else ctx.qk_rhd_step(dt)
+        single = ctx.get_all(I.FIELDS[:9])
+        info1 = ctx.qk_last_info()
+    parts = _run_decomposed(params, fields, world, nsteps, kind)
+    for name in (I.FIELDS[:5] if kind == "hydro" else I.FIELDS[:9]):
+        glued = np.concatenate([parts[r][0][name] for r in range(world)], axis=0)
+        assert np.array_equal(glued, single[name]), name
+    assert all(p[2] > 0 for p in parts)                     # the exchange really ran
+    if kind == "rhd":
+        assert sum(p[1]["newton_total_iters"] for p in parts) == info1["newton_total_iters"]
