@@ -22,6 +22,7 @@ NG = 4
 FIELDS = ["rho", "mx", "my", "mz", "E", "Er", "Fx", "Fy", "Fz", "kappaP", "kappaR"]
 BC_PERIODIC, BC_OUTFLOW = 0, 1
 FLAG_TAU_CORR, FLAG_STATIC_MATTER, FLAG_NEWTON_LITERAL = 1, 2, 4
+FLAG_PLM, FLAG_EDDINGTON = 8, 16
 EOS_IDEAL, EOS_ALPHA_T3 = 0, 1
 FILL_HYDRO, FILL_RAD, FILL_ALL = 1, 2, 7
 
@@ -72,6 +73,8 @@ def lib():
         "orc_nsub_for": (i, [p, d]),
         "orc_cons_to_prim": (None, [d, dp, dp]),
         "orc_ppm_faces": (None, [dp, dp, dp]),
+        "orc_plm_faces": (None, [dp, dp, dp]),
+        "orc_closure_k": (None, [u, dp, i, dp, dp]),
         "orc_mc_slope": (d, [d, d, d]),
         "orc_flatten_1d": (d, [d, dp, dp]),
         "orc_hllc": (None, [d, dp, dp, dp]),

@@ -33,6 +33,21 @@ double orc_mc_slope(double qm1, double q0, double qp1)
     return dc > 0.0 ? lim : -lim;
 }
 
+/* PLM: q_{j-+1/2} = q_j -+ s/2 with s the monotonized-central slope of (q_{j-1}, q_j, q_{j+1}). */
+void orc_plm_faces(const double q[5], double *q_minus, double *q_plus)
+{
+    double s = orc_mc_slope(q[1], q[2], q[3]);
+    *q_minus = q[2] - 0.5 * s;
+    *q_plus = q[2] + 0.5 * s;
+}
+
+/* reconstruction selected by the flags: PPM (default) or PLM */
+void orc_faces(unsigned flags, const double q[5], double *q_minus, double *q_plus)
+{
+    if (flags & ORC_FLAG_PLM) orc_plm_faces(q, q_minus, q_plus);
+    else orc_ppm_faces(q, q_minus, q_plus);
+}
+
 /* Face states of the centre cell q[2] from q[0..4] = q_{j-2..j+2}.
  * (a) eq 22 with each bracket mirror-symmetric about its interface;
  * (b) both states clamped to [min,max] of the cell and its two neighbours;
@@ -186,7 +201,7 @@ static int hydro_divergence(const orc_grid *g, double *const U[5], double *div[5
                     for (int n = 0; n < 5; ++n) {
                         double q[5], qm, qp;
                         for (int m = 0; m < 5; ++m) q[m] = W[n][c + (m - 2) * s];
-                        orc_ppm_faces(q, &qm, &qp);
+                        orc_faces(g->flags, q, &qm, &qp);
                         wl[n][c] = q[2] + chi[c] * (qm - q[2]);    /* flatten toward the average */
                         wr[n][c] = q[2] + chi[c] * (qp - q[2]);
                     }

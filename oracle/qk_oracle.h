@@ -14,6 +14,9 @@
  *        stationary contact, Sod vs exact Riemann solution, advected
  *        wave order, conservation, equilibrium invariance, x<->y symmetry
  *   orc_closure                             : chi(0)=1/3, chi(1)=1, trace T = 1
+ *   orc_plm_faces (ORC_FLAG_PLM)            : exact on linear data, zero slope at extrema, second-order
+ *        advected wave, conservation, contact preservation
+ *   ORC_FLAG_EDDINGTON                      : T = I/3 for every f; linear wave speed c_hat/sqrt(3)
  *   orc_rad_step (transport)                : linear wave speed c_hat/sqrt(3), streaming
  *        top-hat causality/positivity, conservation, split-diffusion factor
  *   orc_exchange_cell                       : eq 57 relaxation to 1e-5,
@@ -36,7 +39,9 @@ extern "C" {
 enum { ORC_RHO = 0, ORC_MX, ORC_MY, ORC_MZ, ORC_E, ORC_ER, ORC_FX, ORC_FY, ORC_FZ,
        ORC_KP, ORC_KR };
 enum { ORC_BC_PERIODIC = 0, ORC_BC_OUTFLOW = 1 };
-enum { ORC_FLAG_TAU_CORR = 1, ORC_FLAG_STATIC_MATTER = 2, ORC_FLAG_NEWTON_LITERAL = 4 };
+enum { ORC_FLAG_TAU_CORR = 1, ORC_FLAG_STATIC_MATTER = 2, ORC_FLAG_NEWTON_LITERAL = 4,
+       ORC_FLAG_PLM = 8,          /* piecewise-linear reconstruction with the MC limiter */
+       ORC_FLAG_EDDINGTON = 16 }; /* Eddington approximation chi = 1/3 (P_r = E_r/3)  */
 enum { ORC_EOS_IDEAL = 0, ORC_EOS_ALPHA_T3 = 1 };   /* eq 55, PAPER.md:424 (oracle only) */
 enum { ORC_FILL_HYDRO = 1, ORC_FILL_RAD = 2, ORC_FILL_ALL = 7 }; /* bit 4: opacities */
 
@@ -86,11 +91,14 @@ int    orc_nsub_for(const orc_grid *g, double dt);
 /* building blocks, exported so the pins can reach them one by one */
 void   orc_cons_to_prim(double gamma, const double U[5], double W[5]);
 void   orc_ppm_faces(const double q[5], double *q_minus, double *q_plus);
+void   orc_plm_faces(const double q[5], double *q_minus, double *q_plus);
+void   orc_faces(unsigned flags, const double q[5], double *q_minus, double *q_plus);
 double orc_mc_slope(double qm1, double q0, double qp1);
 double orc_flatten_1d(double gamma, const double P[5], const double vn[5]);
 void   orc_hllc(double gamma, const double WL[5], const double WR[5], double F[5]);
 double orc_eddington_factor(double f);
 void   orc_closure(const double fvec[3], int n, double T_col[3], double *chi_out);
+void   orc_closure_k(unsigned flags, const double fvec[3], int n, double T_col[3], double *chi_out);
 void   orc_rad_phys_flux(double c, double c_hat, const double S[4], int n, double G[4], double *Tnn);
 int    orc_rad_hll(double c, double c_hat, const double SL[4], const double SR[4], int n,
                    double tau_face, unsigned flags, double G[4]);

@@ -35,6 +35,31 @@ void orc_closure(const double fvec[3], int n, double T_col[3], double *chi_out)
     if (chi_out) *chi_out = chi;
 }
 
+/* closure selected by the flags: Levermore (eq 23-25, default) or the Eddington approximation chi = 1/3,
+ * i.e. P_r = E_r/3 I whatever the flux ("any local closure f -> chi") */
+void orc_closure_k(unsigned flags, const double fvec[3], int n, double T_col[3], double *chi_out)
+{
+    if (flags & ORC_FLAG_EDDINGTON) {
+        double chi = 1.0 / 3.0;
+        double a = 0.5 * (1.0 - chi);
+        for (int i = 0; i < 3; ++i) T_col[i] = (i == n) ? a : 0.0;     /* (3chi-1)/2 = 0: no n n term */
+        if (chi_out) *chi_out = chi;
+        return;
+    }
+    orc_closure(fvec, n, T_col, chi_out);
+}
+
+static void rad_phys_flux_k(unsigned flags, double c, double c_hat, const double S[4], int n, double G[4], double *Tnn)
+{
+    double T[3];
+    orc_closure_k(flags, &S[1], n, T, NULL);
+    double Fn = (c * S[0]) * S[1 + n];
+    double cc = (c * c_hat) * S[0];
+    G[0] = (c_hat / c) * Fn;
+    for (int i = 0; i < 3; ++i) G[1 + i] = cc * T[i];
+    if (Tnn) *Tnn = T[n];
+}
+
 /* Physical flux through a face with normal n of the state S = (E_r, f_x, f_y, f_z):
  * (c_hat/c) F_n for E_r and c c_hat E_r T_in for F_i (eq 11-12). */
 void orc_rad_phys_flux(double c, double c_hat, const double S[4], int n, double G[4], double *Tnn)
@@ -58,8 +83,8 @@ int orc_rad_hll(double c, double c_hat, const double SL[4], const double SR[4], 
                 double tau_face, unsigned flags, double G[4])
 {
     double GL[4], GR[4], TL, TR;
-    orc_rad_phys_flux(c, c_hat, SL, n, GL, &TL);
-    orc_rad_phys_flux(c, c_hat, SR, n, GR, &TR);
+    rad_phys_flux_k(flags, c, c_hat, SL, n, GL, &TL);
+    rad_phys_flux_k(flags, c, c_hat, SR, n, GR, &TR);
     double S = max2(max2(c_hat * sqrt(TL), c_hat * sqrt(TR)), 0.1 * c_hat);
     double UL[4] = { SL[0], (c * SL[0]) * SL[1], (c * SL[0]) * SL[2], (c * SL[0]) * SL[3] };
     double UR[4] = { SR[0], (c * SR[0]) * SR[1], (c * SR[0]) * SR[2], (c * SR[0]) * SR[3] };
@@ -128,7 +153,7 @@ static int rad_divergence(orc_grid *g, double *const R[4], double *div[4])
                     for (int m = 0; m < 4; ++m) {
                         double q[5];
                         for (int t = 0; t < 5; ++t) q[t] = S[m][c + (t - 2) * s];
-                        orc_ppm_faces(q, &lo4[m], &hi4[m]);      /* no flattening */
+                        orc_faces(g->flags, q, &lo4[m], &hi4[m]); /* no flattening */
                     }
                     /* first-order fallback per face state when |f|>1 (or E_r<=0) */
                     double f2 = (lo4[1] * lo4[1] + lo4[2] * lo4[2]) + lo4[3] * lo4[3];

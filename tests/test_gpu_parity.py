@@ -352,6 +352,16 @@ def test_rhd_config4_full_size_sampled():
                        I.FIELDS[:9], P.TOL_ONE_STEP, halo=14, core=4, nsamples=3)
 
 
+@pytest.mark.gpu
+@pytest.mark.slow
+def test_rhd_config5_512_sampled():
+    """BASELINE.json configs[4] (512^3 coupled RHD, 50.6 GB of device state): one full cycle, sampled.
+    Opt-in (QK_SLOW=1): the host-side input generation alone takes minutes."""
+    params, fields = I.config5()
+    _sampled_full_size(params, fields, lambda c, dt: c.qk_rhd_step(dt), lambda g, dt: g.rhd_step(dt),
+                       I.FIELDS[:9], P.TOL_ONE_STEP, halo=14, core=4, nsamples=3)
+
+
 # ------------------------------------------------------------------------------------------------
 # 8(e): z-slab decomposition -- two slabs (two contexts, two host threads, one GPU) against one box
 # ------------------------------------------------------------------------------------------------
