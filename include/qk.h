@@ -44,7 +44,12 @@ enum { QK_RHO = 0, QK_MX, QK_MY, QK_MZ, QK_E, QK_ER, QK_FX, QK_FY, QK_FZ, QK_KAP
 
 enum { QK_FLAG_TAU_CORR = 1,        /* guarded optical-depth correction of the E_r HLL flux (R6) */
        QK_FLAG_STATIC_MATTER = 2,   /* exchange skips eq 41-43: gas held at rest (X11)            */
-       QK_FLAG_NEWTON_LITERAL = 4 };/* literal stop rule of PAPER.md:237 instead of converge-then-polish (X5)   */
+       QK_FLAG_NEWTON_LITERAL = 4,  /* literal stop rule of PAPER.md:237 instead of converge-then-polish (X5)   */
+       /* scheme variants (sweep path only; QK_EINVAL from the step calls on the cross-check paths): */
+       QK_FLAG_PLM = 8,             /* piecewise-linear reconstruction, monotonized-central limiter, for hydro
+                                       and radiation instead of PPM                              */
+       QK_FLAG_EDDINGTON = 16 };    /* Eddington approximation chi = 1/3, P_r = E_r/3,
+                                       instead of the Levermore closure                                         */
 
 enum { QK_FILL_HYDRO = 1, QK_FILL_RAD = 2, QK_FILL_OPACITY = 4, QK_FILL_ALL = 7 };
 

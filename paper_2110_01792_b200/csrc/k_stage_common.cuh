@@ -120,6 +120,19 @@ __device__ __forceinline__ void ppm_lockstep(Q q, double lo[NV], double hi[NV])
     }
 }
 
+// PLM: face states q -+ s/2 with the monotonized-central slope of the three cell averages
+template <int NV, typename Q>
+__device__ __forceinline__ void plm_states(Q q, double lo[NV], double hi[NV])
+{
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+        const double c = q(v, 2);
+        const double s = mc_slope(q(v, 1), c, q(v, 3));
+        lo[v] = c - 0.5 * s;
+        hi[v] = c + 0.5 * s;
+    }
+}
+
 // flattened PPM face states of all five primitives of one cell; q(v, m) = value of variable v at
 // stencil offset m-2
 template <int BL = 0, typename Q>

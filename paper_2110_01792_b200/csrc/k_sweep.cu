@@ -31,18 +31,21 @@ __device__ __noinline__ Flux5 hllc_flux_slow(double gamma, double rL, double uL,
     return hllc_flux(gamma, rL, uL, vL, wL, pL, rR, uR, vR, wR, pR);
 }
 
+template <int CL>
 __device__ __noinline__ Rad4 rad_hll_flux_slow(double c, double c_hat, double EL, double fxL, double fyL, double fzL,
                                                double ER, double fxR, double fyR, double fzR, int n, double tau,
                                                bool tau_corr, int *guard)
 {
     int gd;
-    const Rad4 G = rad_hll_flux(c, c_hat, EL, fxL, fyL, fzL, ER, fxR, fyR, fzR, n, tau, tau_corr, gd);
+    const Rad4 G = rad_hll_flux<CL>(c, c_hat, EL, fxL, fyL, fzL, ER, fxR, fyR, fzR, n, tau, tau_corr, gd);
     *guard = gd;
     return G;
 }
 
 // ---- hydro ------------------------------------------------------------------------------------------
-struct HydroPh {
+// RECON: 0 = PPM, 1 = PLM with the MC limiter
+template <int RECON>
+struct HydroPhT {
     static constexpr int NV = 5;
     static constexpr bool COUNTS = false;
     // select-only PPM limiter (same values): measured faster in the x sweep, slower in the marching sweeps
@@ -59,7 +62,18 @@ struct HydroPh {
     template <int BL, class Q>
     __device__ __forceinline__ int states(Q q, double x, double lo[5], double hi[5]) const
     {
-        ppm_cell<BL>(q, x, lo, hi);
+        if (RECON == 1) {
+            double l[5], h[5];
+            plm_states<5>(q, l, h);
+#pragma unroll
+            for (int v = 0; v < 5; ++v) {
+                const double c = q(v, 2);
+                lo[v] = c + x * (l[v] - c);         // flatten toward the cell average
+                hi[v] = c + x * (h[v] - c);
+            }
+        } else {
+            ppm_cell<BL>(q, x, lo, hi);
+        }
         return 0;
     }
     // MODE 2 epilogue: primitives of the updated cell for the next stage's sweeps and,
@@ -112,7 +126,9 @@ struct HydroPh {
 };
 
 // ---- radiation --------------------------------------------------------------------------------------
-struct RadPh {
+// RECON as for hydro; CL: 0 = Levermore closure (eq 23-25), 1 = Eddington approximation
+template <int RECON, int CL>
+struct RadPhT {
     static constexpr int NV = 4;
     static constexpr bool COUNTS = true;
     static constexpr int BL_X = QK_BLX_R, BL_MARCH = QK_BLM_R;
@@ -136,7 +152,22 @@ struct RadPh {
     template <int BL, class Q>
     __device__ __forceinline__ int states(Q q, double, double lo[4], double hi[4]) const
     {
-        return rad_ppm_cell<BL>(q, lo, hi);
+        if (RECON == 0) return rad_ppm_cell<BL>(q, lo, hi);
+        plm_states<4>(q, lo, hi);
+        int nfall = 0;      // first-order fallback per face state, as in rad_ppm_cell
+        double f2 = (lo[1] * lo[1] + lo[2] * lo[2]) + lo[3] * lo[3];
+        if (f2 > 1.0 || !(lo[0] > 0.0)) {
+#pragma unroll
+            for (int v = 0; v < 4; ++v) lo[v] = q(v, 2);
+            ++nfall;
+        }
+        f2 = (hi[1] * hi[1] + hi[2] * hi[2]) + hi[3] * hi[3];
+        if (f2 > 1.0 || !(hi[0] > 0.0)) {
+#pragma unroll
+            for (int v = 0; v < 4; ++v) hi[v] = q(v, 2);
+            ++nfall;
+        }
+        return nfall;
     }
     // MODE 2 epilogue: (E_r, f = F_r / (c E_r)) of the updated cell, as rad_prim_kernel
     struct Tail { int bad = 0; };
@@ -164,9 +195,9 @@ struct RadPh {
 #else
         unsigned risk = 0;
         int guard;
-        Rad4 g = rad_hll_flux_fast(c, c_hat, L[0], L[1], L[2], L[3], R[0], R[1], R[2], R[3], DIR, tau, tau_corr != 0,
+        Rad4 g = rad_hll_flux_fast<CL>(c, c_hat, L[0], L[1], L[2], L[3], R[0], R[1], R[2], R[3], DIR, tau, tau_corr != 0,
                                    guard, risk);
-        if (risk) g = rad_hll_flux_slow(c, c_hat, L[0], L[1], L[2], L[3], R[0], R[1], R[2], R[3], DIR, tau,
+        if (risk) g = rad_hll_flux_slow<CL>(c, c_hat, L[0], L[1], L[2], L[3], R[0], R[1], R[2], R[3], DIR, tau,
                                         tau_corr != 0, &guard);
         G[0] = g.e; G[1] = g.x; G[2] = g.y; G[3] = g.z;
         return guard;
@@ -258,31 +289,37 @@ static int launch_sweeps(const PH &ph, const Geom &g, double dtdx, int stage, Fi
     return n;
 }
 
-int launch_hydro_sweeps(const Geom &g, double gamma, double dtdx, int stage, CHydro5 W, const double *chi, Hydro5 D,
-                        CHydro5 U, CHydro5 U0, Hydro5 out, Hydro5 Wout, Counters *ctr, StateCache *cache, cudaStream_t st,
-                        int which)
+int launch_hydro_sweeps(const Geom &g, double gamma, unsigned scheme, double dtdx, int stage, CHydro5 W,
+                        const double *chi, Hydro5 D, CHydro5 U, CHydro5 U0, Hydro5 out, Hydro5 Wout, Counters *ctr,
+                        StateCache *cache, cudaStream_t st, int which)
 {
-    HydroPh ph;
-    ph.w[0] = W.rho; ph.w[1] = W.mx; ph.w[2] = W.my; ph.w[3] = W.mz; ph.w[4] = W.E;
-    ph.chi = chi; ph.gamma = gamma;
     FieldsRW<5> d{{D.rho, D.mx, D.my, D.mz, D.E}}, o{{out.rho, out.mx, out.my, out.mz, out.E}};
     FieldsRO<5> u{{U.rho, U.mx, U.my, U.mz, U.E}}, u0{{U0.rho, U0.mx, U0.my, U0.mz, U0.E}};
     FieldsRW<5> wo{{Wout.rho, Wout.mx, Wout.my, Wout.mz, Wout.E}};
-    return launch_sweeps(ph, g, dtdx, stage, d, u, u0, o, wo, ctr, cache, st, which);
+    auto go = [&](auto ph) {
+        ph.w[0] = W.rho; ph.w[1] = W.mx; ph.w[2] = W.my; ph.w[3] = W.mz; ph.w[4] = W.E;
+        ph.chi = chi; ph.gamma = gamma;
+        return launch_sweeps(ph, g, dtdx, stage, d, u, u0, o, wo, ctr, cache, st, which);
+    };
+    return (scheme & QK_FLAG_PLM) ? go(HydroPhT<1>()) : go(HydroPhT<0>());
 }
 
 int launch_rad_sweeps(const Geom &g, const PhysConsts &pc, double dtdx, int stage, CRad4p S, const double *rho,
                       const double *kappaR, Rad4p D, CRad4p R, CRad4p R0, Rad4p out, Rad4p Sout, Counters *ctr,
                       cudaStream_t st, int which)
 {
-    RadPh ph;
-    ph.s[0] = S.E; ph.s[1] = S.Fx; ph.s[2] = S.Fy; ph.s[3] = S.Fz;
-    ph.rho = rho; ph.kR = kappaR;
-    ph.c = pc.c; ph.c_hat = pc.c_hat; ph.dx = pc.dx; ph.tau_corr = (pc.flags & QK_FLAG_TAU_CORR) ? 1 : 0;
     FieldsRW<4> d{{D.E, D.Fx, D.Fy, D.Fz}}, o{{out.E, out.Fx, out.Fy, out.Fz}};
     FieldsRO<4> u{{R.E, R.Fx, R.Fy, R.Fz}}, u0{{R0.E, R0.Fx, R0.Fy, R0.Fz}};
     FieldsRW<4> so{{Sout.E, Sout.Fx, Sout.Fy, Sout.Fz}};
-    return launch_sweeps(ph, g, dtdx, stage, d, u, u0, o, so, ctr, nullptr, st, which);
+    auto go = [&](auto ph) {
+        ph.s[0] = S.E; ph.s[1] = S.Fx; ph.s[2] = S.Fy; ph.s[3] = S.Fz;
+        ph.rho = rho; ph.kR = kappaR;
+        ph.c = pc.c; ph.c_hat = pc.c_hat; ph.dx = pc.dx; ph.tau_corr = (pc.flags & QK_FLAG_TAU_CORR) ? 1 : 0;
+        return launch_sweeps(ph, g, dtdx, stage, d, u, u0, o, so, ctr, nullptr, st, which);
+    };
+    const bool plm = (pc.flags & QK_FLAG_PLM) != 0, edd = (pc.flags & QK_FLAG_EDDINGTON) != 0;
+    if (plm) return edd ? go(RadPhT<1, 1>()) : go(RadPhT<1, 0>());
+    return edd ? go(RadPhT<0, 1>()) : go(RadPhT<0, 0>());
 }
 
 }  // namespace qk

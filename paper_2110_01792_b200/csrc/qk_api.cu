@@ -230,7 +230,7 @@ void hydro_stage_sweep(qk_ctx *c, double dtdx, int stage, double *const *U, doub
     }
     for (int d = 0; d < 3; ++d) {
         Scope s(c, K_HYDRO_SWEEP_X + d);
-        s.done(launch_hydro_sweeps(g, c->pc.gamma, dtdx, stage, ch5(W), c->chi, h5(D), ch5(U), ch5(U0), h5(out), h5(Wout),
+        s.done(launch_hydro_sweeps(g, c->pc.gamma, c->pc.flags, dtdx, stage, ch5(W), c->chi, h5(D), ch5(U), ch5(U0), h5(out), h5(Wout),
                                    c->ctr, c->cache, c->stream, 1 << d));
     }
 }
@@ -242,8 +242,15 @@ void hydro_stage(qk_ctx *c, double dtdx, int stage, double *const *U, double *co
     else hydro_stage_unfused(c, dtdx, stage, U, U0, out);
 }
 
+// the PLM / Eddington variants exist in the sweep path only
+bool scheme_supported(const qk_ctx *c)
+{
+    return c->path == QK_PATH_SWEEP || !(c->pc.flags & (QK_FLAG_PLM | QK_FLAG_EDDINGTON));
+}
+
 int do_hydro_step(qk_ctx *c, double dt)
 {
+    if (!scheme_supported(c)) return QK_EINVAL;
     const double dtdx = dt / c->pc.dx;
     double *const *Un = &c->state[QK_RHO];
     double *const *U1 = &c->stage[0];
@@ -324,6 +331,7 @@ void rad_stage(qk_ctx *c, double dtdx, int stage, double *const *R, double *cons
 
 int do_rad_transport(qk_ctx *c, double dt)
 {
+    if (!scheme_supported(c)) return QK_EINVAL;
     const double dtdx = dt / c->pc.dx;
     double *const *Rn = &c->state[QK_ER];
     double *const *R1 = &c->stage[0];

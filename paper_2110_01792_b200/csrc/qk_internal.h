@@ -92,9 +92,9 @@ int launch_rad_stage(const Geom &g, const PhysConsts &pc, double dtdx, int stage
                      const double *kappaR, Rad4p out, Counters *ctr, cudaStream_t st);
 
 // sweep path (k_sweep.cu); `which` bit 0 = x sweep, bit 1 = y sweep, bit 2 = z sweep + RK update
-int launch_hydro_sweeps(const Geom &g, double gamma, double dtdx, int stage, CHydro5 W, const double *chi, Hydro5 D,
-                        CHydro5 U, CHydro5 U0, Hydro5 out, Hydro5 Wout, Counters *ctr, StateCache *cache, cudaStream_t st,
-                        int which);
+int launch_hydro_sweeps(const Geom &g, double gamma, unsigned scheme, double dtdx, int stage, CHydro5 W,
+                        const double *chi, Hydro5 D, CHydro5 U, CHydro5 U0, Hydro5 out, Hydro5 Wout, Counters *ctr,
+                        StateCache *cache, cudaStream_t st, int which);
 int launch_chi_two_pass(const Geom &g, double gamma, CHydro5 W, double *cx, double *cy, double *cz, double *chi,
                         cudaStream_t st);
 int launch_rad_sweeps(const Geom &g, const PhysConsts &pc, double dtdx, int stage, CRad4p S, const double *rho,

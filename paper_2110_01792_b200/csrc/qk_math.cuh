@@ -185,12 +185,14 @@ QK_HD double eddington_factor(double f)
 // n = f/|f| (eq 25), isotropic when f = 0.  Returns T_nn in Tnn.
 struct Rad4 { double e, x, y, z; };
 
+// CL = closure: 0 Levermore (eq 24), 1 Eddington approximation chi = 1/3 (the n n term vanishes)
+template <int CL = 0>
 QK_HD Rad4 rad_physical_flux(double c, double c_hat, double E, double fx, double fy, double fz, int n,
                              double &Tnn)
 {
     const double fsq = (fx * fx + fy * fy) + fz * fz;
-    const double fmag = sqrt(fsq);
-    const double chi = eddington_factor(lesser(fmag, 1.0));
+    const double fmag = CL == 1 ? 0.0 : sqrt(fsq);
+    const double chi = CL == 1 ? 1.0 / 3.0 : eddington_factor(lesser(fmag, 1.0));
     const double iso = 0.5 * (1.0 - chi), aniso = 0.5 * (3.0 * chi - 1.0);
     double Tx = (n == 0) ? iso : 0.0, Ty = (n == 1) ? iso : 0.0, Tz = (n == 2) ? iso : 0.0;
     if (fmag > 0.0) {
@@ -216,13 +218,14 @@ QK_HD Rad4 rad_physical_flux(double c, double c_hat, double E, double fx, double
 // max(c_hat sqrt(Tnn_L), c_hat sqrt(Tnn_R), 0.1 c_hat) (R5); the E_r
 // dissipation is scaled by min(1, 1/tau_face) (R6) unless a star state it
 // implies is non-causal.  `guard` is set to 1 when the correction was disabled for the face.
+template <int CL = 0>
 QK_HD Rad4 rad_hll_flux(double c, double c_hat, double EL, double fxL, double fyL, double fzL,
                         double ER, double fxR, double fyR, double fzR, int n, double tau_face,
                         bool tau_corr, int &guard)
 {
     double TL, TR;
-    const Rad4 GL = rad_physical_flux(c, c_hat, EL, fxL, fyL, fzL, n, TL);
-    const Rad4 GR = rad_physical_flux(c, c_hat, ER, fxR, fyR, fzR, n, TR);
+    const Rad4 GL = rad_physical_flux<CL>(c, c_hat, EL, fxL, fyL, fzL, n, TL);
+    const Rad4 GR = rad_physical_flux<CL>(c, c_hat, ER, fxR, fyR, fzR, n, TR);
     const double S = greater(greater(c_hat * sqrt(TL), c_hat * sqrt(TR)), 0.1 * c_hat);
     const double FxL = (c * EL) * fxL, FyL = (c * EL) * fyL, FzL = (c * EL) * fzL;
     const double FxR = (c * ER) * fxR, FyR = (c * ER) * fyR, FzR = (c * ER) * fzR;

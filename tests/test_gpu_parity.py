@@ -222,6 +222,68 @@ def test_rad_transport_config3_small(path):
     g.close()
 
 
+# ------------------------------------------------------------------------------------------------
+# 8(f) NEXT-1: PLM reconstruction and the Eddington-approximation closure (sweep path)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bc", [B.QK_BC_PERIODIC, B.QK_BC_OUTFLOW], ids=["periodic", "outflow"])
+def test_hydro_plm_ragged_shocks(bc):
+    params, fields = I.ragged_hydro(bc=bc)
+    params["flags"] = I.FLAG_TAU_CORR | I.FLAG_PLM
+    res = _run_hydro_pair(params, fields, 5, B.QK_PATH_SWEEP, check_at=(1,))
+    P.assert_parity(*res[1], P.TOL_ONE_STEP, P.HYDRO, "PLM step 1")
+    P.assert_parity(*res[5], P.TOL_100_STEPS, P.HYDRO, "PLM step 5")
+    # and it is a different scheme from PPM
+    params["flags"] = I.FLAG_TAU_CORR
+    ppm = _run_hydro_pair(params, fields, 1, B.QK_PATH_SWEEP)
+    assert not np.array_equal(ppm[1][1]["rho"], res[1][1]["rho"])
+
+
+@pytest.mark.parametrize("variant", [I.FLAG_PLM, I.FLAG_EDDINGTON, I.FLAG_PLM | I.FLAG_EDDINGTON],
+                         ids=["plm", "eddington", "plm+eddington"])
+def test_rad_transport_variants_config3_small(variant):
+    params, fields = I.config3(shape=(24, 20, 28))
+    params["flags"] |= variant
+    if variant & I.FLAG_EDDINGTON:      # P_r = E_r/3 cannot carry the generator's f ~ 0.9 noise (E_r goes negative)
+        for n in ("Fx", "Fy", "Fz"):
+            fields[n] = 0.3 * fields[n]
+    g = P.make_oracle(params, fields)
+    dt = 0.3 * params["dx"] / params["c_hat"]
+    with P.make_gpu(params, fields) as ctx:
+        for s in range(1, 6):
+            assert g.rad_transport(dt) == 0
+            ctx.qk_rad_transport(dt)
+            io, ig = g.info(), ctx.qk_last_info()
+            assert ig["fallback_states"] == io["fallback_states"] and ig["guard_faces"] == io["guard_faces"], s
+            if s == 1:
+                P.assert_parity(g.get_all(RADF), ctx.get_all(RADF), P.TOL_ONE_STEP, P.RAD, "rad variant step 1")
+        P.assert_parity(g.get_all(RADF), ctx.get_all(RADF), P.TOL_100_STEPS, P.RAD, "rad variant step 5")
+    g.close()
+
+
+def test_rhd_step_plm_eddington_ragged():
+    params, fields = I.ragged_rhd()
+    params["flags"] = I.FLAG_TAU_CORR | I.FLAG_PLM | I.FLAG_EDDINGTON
+    g = P.make_oracle(params, fields)
+    with P.make_gpu(params, fields) as ctx:
+        for s in range(3):
+            dt = g.cfl_dt()
+            assert ctx.qk_cfl_dt() == dt
+            assert g.rhd_step(dt) == 0
+            ctx.qk_rhd_step(dt)
+        names = I.FIELDS[:9]
+        P.assert_parity(g.get_all(names), ctx.get_all(names), P.TOL_100_STEPS, None, "PLM+Eddington RHD step 3")
+        assert ctx.qk_last_info()["newton_total_iters"] == g.info()["newton_total_iters"]
+    g.close()
+
+
+def test_variants_rejected_on_cross_check_paths():
+    params, fields = I.ragged_hydro()
+    params["flags"] = I.FLAG_TAU_CORR | I.FLAG_PLM
+    with P.make_gpu(params, fields, path=B.QK_PATH_FUSED) as ctx:
+        with pytest.raises(B.QkError):
+            ctx.qk_hydro_step(1e-4)
+
+
 @pytest.mark.parametrize("flags", [1, 3, 5], ids=["default", "static_matter", "literal_stop"])
 def test_exchange_parity_and_counters(flags):
     params, fields = I.ragged_rhd()
