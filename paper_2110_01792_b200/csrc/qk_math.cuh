@@ -106,12 +106,16 @@ QK_HD void ppm_face_states(double a, double b, double c, double d, double e, dou
 QK_HD double flatten_coeff_1d(double gamma, double Pm2, double Pm1, double P0, double Pp1, double Pp2,
                               double vn_m1, double vn_p1)
 {
+    if (!(vn_p1 < vn_m1)) return 1.0;          // expanding flow: nothing below is needed
     const double near = fabs(Pp1 - Pm1);
+    // Weak jump: near < 0.2499 gamma P0 makes near / (gamma P0) < 0.25, hence (0.75 - strength) / 0.5 > 1, its
+    // clamp exactly 1 and the result max(steep, 1) = 1 whatever `steep` is -- the value the full evaluation
+    // below returns, without its three divisions.  (Only genuine shocks get past this line.)
+    if (near < 0.2499 * (gamma * P0)) return 1.0;
     const double far = fabs(Pp2 - Pm2);
     double steep;
     if (far == 0.0) steep = (near == 0.0) ? 1.0 : 0.0;
     else            steep = unit_clamp((0.85 - near / far) / 0.10);
-    if (!(vn_p1 < vn_m1)) return 1.0;
     const double strength = near / (gamma * P0);
     return greater(steep, unit_clamp((0.75 - strength) / 0.5));
 }
