@@ -88,16 +88,33 @@ void orc_get_info(const orc_grid *g, long long *out7)
     out7[6] = g->guard_faces;
 }
 
-/* source index along one axis for a ghost index (PAPER.md:293,572 periodic; 464 outflow).
- * Outflow is read as zero-gradient: copy of the nearest interior cell (H15). */
+/* source index along one axis for a ghost index (PAPER.md:293,572 periodic; 464 outflow; 408 reflecting).
+ * Outflow is read as zero-gradient: copy of the nearest interior cell (H15).
+ * Reflecting: the mirror image about the wall, ghost -1 <- cell 0, -2 <- 1, n <- n-1, ... (B1). */
 static int src_index(int i, int n, int bc)
 {
     if (i >= 0 && i < n) return i;
     if (bc == ORC_BC_PERIODIC) { int m = i % n; if (m < 0) m += n; return m; }
+    if (bc == ORC_BC_REFLECTING) {
+        int m = i < 0 ? -1 - i : 2 * n - 1 - i;
+        return m < 0 ? 0 : (m > n - 1 ? n - 1 : m);        /* boxes thinner than the ghost width */
+    }
     return i < 0 ? 0 : n - 1;
 }
 
-static void fill_one(orc_grid *g, double *a)
+/* vector component a field carries (0,1,2) or -1 for a scalar: at a reflecting wall normal to axis a the
+ * a-component of the momentum and of the radiation flux changes sign in the image cell */
+static int field_component(int field)
+{
+    switch (field) {
+    case ORC_MX: case ORC_FX: return 0;
+    case ORC_MY: case ORC_FY: return 1;
+    case ORC_MZ: case ORC_FZ: return 2;
+    default: return -1;
+    }
+}
+
+static void fill_one(orc_grid *g, double *a, int comp)
 {
     /* every ghost cell (faces, edges, corners) <- the interior cell its three axis
      * indices map to; equivalent to filling x, then y, then z in sequence. */
@@ -108,19 +125,25 @@ static void fill_one(orc_grid *g, double *a)
             for (int i = -ORC_NG; i < g->nx + ORC_NG; ++i) {
                 int is = src_index(i, g->nx, g->bc);
                 if (is == i && js == j && ks == k) continue;
-                a[idx(g, i, j, k)] = a[idx(g, is, js, ks)];
+                double v = a[idx(g, is, js, ks)];
+                if (g->bc == ORC_BC_REFLECTING) {
+                    int outside = (comp == 0 && (i < 0 || i >= g->nx)) || (comp == 1 && (j < 0 || j >= g->ny)) ||
+                                  (comp == 2 && (k < 0 || k >= g->nz));
+                    if (outside) v = -v;
+                }
+                a[idx(g, i, j, k)] = v;
             }
         }
     }
 }
 
-void orc_fill_field(orc_grid *g, int field) { fill_one(g, g->f[field]); }
+void orc_fill_field(orc_grid *g, int field) { fill_one(g, g->f[field], field_component(field)); }
 
 void orc_fill_boundary(orc_grid *g, int which)
 {
-    if (which & ORC_FILL_HYDRO) for (int f = ORC_RHO; f <= ORC_E; ++f) fill_one(g, g->f[f]);
-    if (which & ORC_FILL_RAD)   for (int f = ORC_ER; f <= ORC_FZ; ++f) fill_one(g, g->f[f]);
-    if (which & 4)              for (int f = ORC_KP; f <= ORC_KR; ++f) fill_one(g, g->f[f]);
+    if (which & ORC_FILL_HYDRO) for (int f = ORC_RHO; f <= ORC_E; ++f) fill_one(g, g->f[f], field_component(f));
+    if (which & ORC_FILL_RAD)   for (int f = ORC_ER; f <= ORC_FZ; ++f) fill_one(g, g->f[f], field_component(f));
+    if (which & 4)              for (int f = ORC_KP; f <= ORC_KR; ++f) fill_one(g, g->f[f], -1);
 }
 
 /* eq 21: dt = CFL dx / max(|v| + c_s), |v| the vector magnitude

@@ -38,7 +38,8 @@ extern "C" {
 
 enum { ORC_RHO = 0, ORC_MX, ORC_MY, ORC_MZ, ORC_E, ORC_ER, ORC_FX, ORC_FY, ORC_FZ,
        ORC_KP, ORC_KR };
-enum { ORC_BC_PERIODIC = 0, ORC_BC_OUTFLOW = 1 };
+enum { ORC_BC_PERIODIC = 0, ORC_BC_OUTFLOW = 1,
+       ORC_BC_REFLECTING = 2 };  /* solid wall: mirror image, normal momentum / flux component negated */
 enum { ORC_FLAG_TAU_CORR = 1, ORC_FLAG_STATIC_MATTER = 2, ORC_FLAG_NEWTON_LITERAL = 4,
        ORC_FLAG_PLM = 8,          /* piecewise-linear reconstruction with the MC limiter */
        ORC_FLAG_EDDINGTON = 16 }; /* Eddington approximation chi = 1/3 (P_r = E_r/3)  */
