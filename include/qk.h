@@ -34,7 +34,9 @@ enum { QK_OK = 0, QK_EINVAL = 1, QK_ENOMEM = 2, QK_ECUDA = 3,
        QK_ESTATE = 5 };  /* rho<=0, P<=0, E_g<=0 or E_r<=0 met (PAPER.md:438 needs E_r>0)      */
 
 enum { QK_BC_PERIODIC = 0,
-       QK_BC_OUTFLOW = 1 };  /* PAPER.md:464; zero-gradient copy of the nearest interior cell (H15) */
+       QK_BC_OUTFLOW = 1,    /* PAPER.md:464; zero-gradient copy of the nearest interior cell (H15) */
+       QK_BC_REFLECTING = 2 };/* PAPER.md:408, 438, 464; solid wall: mirror image, the wall-normal component of
+                                 rho v and F_r negated (B1) */
 
 /* field ids: conserved hydro U=(rho, rho v, E), radiation moments
  * (E_r, F_r) (eq 11-12), Planck- and Rosseland-type opacities per cell

@@ -1,5 +1,6 @@
-// k_boundary.cu -- ghost-zone fill ("B.C. fill"): periodic
-// or outflow = zero-gradient copy of the nearest interior cell (reading H15).
+// k_boundary.cu -- ghost-zone fill ("B.C. fill"): periodic,
+// outflow = zero-gradient copy of the nearest interior cell (reading H15), or reflecting =
+// mirror image with the wall-normal vector component negated (reading B1).
 //
 // Every ghost cell (faces, edges, corners) takes the value of the interior cell its three
 // indices map to, so one pass fills the whole shell with no ordering between directions
@@ -19,6 +20,10 @@ __device__ __forceinline__ int wrap_index(int i, int n, int bc)
     if (bc == QK_BC_PERIODIC) {
         int m = i % n;
         return m < 0 ? m + n : m;
+    }
+    if (bc == QK_BC_REFLECTING) {      // mirror image about the wall: -1 <- 0, -2 <- 1, n <- n-1, ... (B1)
+        const int m = i < 0 ? -1 - i : 2 * n - 1 - i;
+        return m < 0 ? 0 : (m > n - 1 ? n - 1 : m);
     }
     return i < 0 ? 0 : n - 1;
 }
@@ -59,6 +64,17 @@ __global__ void __launch_bounds__(256) fill_ghost_kernel(Geom g, int bc, unsigne
         const int dst = g.at(i, j, k);
         const int src = g.at(wrap_index(i, g.nx, bc), wrap_index(j, g.ny, bc), k_ext ? k : wrap_index(k, g.nz, bc));
         if (src == dst) continue;
+        if (bc == QK_BC_REFLECTING) {
+            // the normal component of rho v / v / F_r / f changes sign across each wall the image lies beyond
+            const bool out[3] = {i < 0 || i >= g.nx, j < 0 || j >= g.ny, !k_ext && (k < 0 || k >= g.nz)};
+#pragma unroll 1
+            for (int f = 0; f < fl.n; ++f) {
+                const double v = fl.f[f][src];
+                const int cm = fl.comp[f];
+                fl.f[f][dst] = (cm >= 0 && out[cm]) ? -v : v;
+            }
+            continue;
+        }
 #pragma unroll 1
         for (int f = 0; f < fl.n; ++f) fl.f[f][dst] = fl.f[f][src];
     }

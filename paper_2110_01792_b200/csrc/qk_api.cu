@@ -160,11 +160,16 @@ CRad4p cr4(double *const *f) { return CRad4p{f[0], f[1], f[2], f[3]}; }
 
 void reset_counters(qk_ctx *c) { cudaMemsetAsync(c->ctr, 0, sizeof(Counters), c->stream); }
 
-void fill_fields(qk_ctx *c, double *const *fields, int n)
+// Every list the drivers fill is (scalar, x, y, z component, scalars ...): U, W, R, S, optionally followed by rho
+// and kappa_R; qk_fill_boundary passes the components of its own list.
+void fill_fields(qk_ctx *c, double *const *fields, int n, const signed char *comps = nullptr)
 {
     FillList fl;
     fl.n = n;
-    for (int i = 0; i < n; ++i) fl.f[i] = fields[i];
+    for (int i = 0; i < n; ++i) {
+        fl.f[i] = fields[i];
+        fl.comp[i] = comps ? comps[i] : (signed char)((i >= 1 && i <= 3) ? i - 1 : -1);
+    }
     Scope s(c, K_FILL);
     if (c->ext_faces && c->halo_fn) {      // neighbours' planes first, then the x / y images of everything
         c->pending = fl;
@@ -217,7 +222,7 @@ void hydro_stage_sweep(qk_ctx *c, double dtdx, int stage, double *const *U, doub
     const Geom &g = c->g;
     double *const *D = &c->scratch[SC_D];
     if (w_ready) {
-        fill_fields(c, W, 5);            // periodic / outflow images commute with the pointwise cons -> prim map
+        fill_fields(c, W, 5);            // periodic / outflow / mirror images commute with the pointwise cons -> prim map
     } else {
         fill_fields(c, U, 5);
         Scope s(c, K_PRIM);
@@ -396,7 +401,7 @@ int qk_init(int nx, int ny, int nz, double dx, double gamma, double c_hat, doubl
     if (!out) return QK_EINVAL;
     *out = nullptr;
     if (nx < 1 || ny < 1 || nz < 1 || !(dx > 0.0) || !(gamma > 1.0) || c_hat < 0.0 || c < 0.0) return QK_EINVAL;
-    if (boundary != QK_BC_PERIODIC && boundary != QK_BC_OUTFLOW) return QK_EINVAL;
+    if (boundary != QK_BC_PERIODIC && boundary != QK_BC_OUTFLOW && boundary != QK_BC_REFLECTING) return QK_EINVAL;
     if ((long long)(nx + 2 * NG) * (ny + 2 * NG) * (nz + 2 * NG) > 2000000000LL) return QK_EINVAL;
     if (ny + 2 > 65535 || nz + 2 > 65535) return QK_EINVAL;
     int dev = 0;
@@ -521,11 +526,14 @@ int qk_fill_boundary(qk_ctx *c, int which)
     int rc = ensure_storage(c);
     if (rc) return rc;
     double *list[QK_NFIELDS];
+    signed char comps[QK_NFIELDS];
+    static const signed char comp_of[QK_NFIELDS] = {-1, 0, 1, 2, -1, -1, 0, 1, 2, -1, -1};
     int n = 0;
-    if (which & QK_FILL_HYDRO) for (int f = QK_RHO; f <= QK_E; ++f) list[n++] = c->state[f];
-    if (which & QK_FILL_RAD) for (int f = QK_ER; f <= QK_FZ; ++f) list[n++] = c->state[f];
-    if (which & QK_FILL_OPACITY) for (int f = QK_KAPPA_P; f <= QK_KAPPA_R; ++f) list[n++] = c->state[f];
-    fill_fields(c, list, n);
+    auto add = [&](int f) { list[n] = c->state[f]; comps[n] = comp_of[f]; ++n; };
+    if (which & QK_FILL_HYDRO) for (int f = QK_RHO; f <= QK_E; ++f) add(f);
+    if (which & QK_FILL_RAD) for (int f = QK_ER; f <= QK_FZ; ++f) add(f);
+    if (which & QK_FILL_OPACITY) for (int f = QK_KAPPA_P; f <= QK_KAPPA_R; ++f) add(f);
+    fill_fields(c, list, n, comps);
     return check_launch();
 }
 

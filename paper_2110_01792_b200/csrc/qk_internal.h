@@ -70,7 +70,9 @@ struct CHydro5 { const double *rho, *mx, *my, *mz, *E; };
 struct Rad4p { double *E, *Fx, *Fy, *Fz; };
 struct CRad4p { const double *E, *Fx, *Fy, *Fz; };
 
-struct FillList { double *f[QK_NFIELDS]; int n; };
+// comp[i] = vector component field i carries (0, 1, 2) or -1 for a scalar: negated in the image cells of a
+// reflecting wall normal to that axis
+struct FillList { double *f[QK_NFIELDS]; signed char comp[QK_NFIELDS]; int n; };
 
 // ---- launchers (each enqueues on `st`; returns the number of kernels launched) -----------------
 int launch_fill(const Geom &g, int bc, unsigned ext_faces, const FillList &fl, cudaStream_t st);

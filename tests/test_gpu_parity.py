@@ -21,7 +21,7 @@ PATH_IDS = ["fused", "unfused", "sweep"]
 # ------------------------------------------------------------------------------------------------
 # S0/S1: layout and boundary fill -- bit-exact
 # ------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("bc", [B.QK_BC_PERIODIC, B.QK_BC_OUTFLOW])
+@pytest.mark.parametrize("bc", [B.QK_BC_PERIODIC, B.QK_BC_OUTFLOW, B.QK_BC_REFLECTING])
 @pytest.mark.parametrize("shape", [(32, 32, 32), (19, 22, 37), (1, 1, 16), (2, 3, 5), (4, 4, 64), (5, 1, 1)])
 def test_boundary_fill_bit_exact(shape, bc):
     nz, ny, nx = shape
@@ -153,7 +153,8 @@ def test_hydro_config1_hundred_steps():
 
 
 @pytest.mark.parametrize("path", PATHS, ids=PATH_IDS)
-@pytest.mark.parametrize("bc", [B.QK_BC_PERIODIC, B.QK_BC_OUTFLOW], ids=["periodic", "outflow"])
+@pytest.mark.parametrize("bc", [B.QK_BC_PERIODIC, B.QK_BC_OUTFLOW, B.QK_BC_REFLECTING],
+                         ids=["periodic", "outflow", "reflecting"])
 def test_hydro_ragged_shocks(bc, path):
     """Non-cubic box that is not a multiple of any tile size, Mach 1.5 (flattening and all HLLC
     branches active), several tiles plus ragged tails in x, y and z."""
@@ -225,7 +226,8 @@ def test_rad_transport_config3_small(path):
 # ------------------------------------------------------------------------------------------------
 # 8(f) NEXT-1: PLM reconstruction and the Eddington-approximation closure (sweep path)
 # ------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("bc", [B.QK_BC_PERIODIC, B.QK_BC_OUTFLOW], ids=["periodic", "outflow"])
+@pytest.mark.parametrize("bc", [B.QK_BC_PERIODIC, B.QK_BC_OUTFLOW, B.QK_BC_REFLECTING],
+                         ids=["periodic", "outflow", "reflecting"])
 def test_hydro_plm_ragged_shocks(bc):
     params, fields = I.ragged_hydro(bc=bc)
     params["flags"] = I.FLAG_TAU_CORR | I.FLAG_PLM
@@ -317,7 +319,8 @@ def test_exchange_newton_cap_is_reported():
 
 
 @pytest.mark.parametrize("path", PATHS, ids=PATH_IDS)
-@pytest.mark.parametrize("bc", [B.QK_BC_PERIODIC, B.QK_BC_OUTFLOW], ids=["periodic", "outflow"])
+@pytest.mark.parametrize("bc", [B.QK_BC_PERIODIC, B.QK_BC_OUTFLOW, B.QK_BC_REFLECTING],
+                         ids=["periodic", "outflow", "reflecting"])
 def test_rhd_step_ragged(bc, path):
     """Full operator-split cycle (hydro, N_sub x (transport, exchange)) on a ragged box."""
     params, fields = I.ragged_rhd(bc=bc)
@@ -488,7 +491,7 @@ def _run_decomposed(params, fields, world, nsteps, kind):
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("bc", [I.BC_PERIODIC, I.BC_OUTFLOW], ids=["periodic", "outflow"])
+@pytest.mark.parametrize("bc", [I.BC_PERIODIC, I.BC_OUTFLOW, I.BC_REFLECTING], ids=["periodic", "outflow", "reflecting"])
 @pytest.mark.parametrize("kind,world", [("hydro", 2), ("hydro", 3), ("rhd", 2)])
 def test_slab_decomposition_is_bitwise_the_single_box(kind, world, bc):
     params, fields = (I.ragged_hydro(bc=bc) if kind == "hydro" else I.ragged_rhd(bc=bc))
@@ -506,3 +509,27 @@ def test_slab_decomposition_is_bitwise_the_single_box(kind, world, bc):
     assert all(p[2] > 0 for p in parts)                     # the exchange really ran
     if kind == "rhd":
         assert sum(p[1]["newton_total_iters"] for p in parts) == info1["newton_total_iters"]
+
+
+def test_implosion_like_reflecting_box_stays_diagonally_symmetric():
+    """PAPER.md:408 (Liska-Wendroff implosion, reflecting walls): an x<->y-symmetric state stays bitwise symmetric
+    on the GPU too (the library is built without FMA contraction), and equals the oracle."""
+    n = 48
+    x = (np.arange(n) + 0.5) / n
+    X, Y = np.meshgrid(x, x, indexing="xy")
+    inside = X + Y < 0.5
+    gamma = 1.4
+    rho2, P2 = np.where(inside, 0.125, 1.0), np.where(inside, 0.14, 1.0)
+    rep = lambda a: np.ascontiguousarray(np.repeat(a[None], 3, axis=0))      # noqa: E731
+    z = np.zeros((3, n, n))
+    fields = {"rho": rep(rho2), "mx": z, "my": z.copy(), "mz": z.copy(), "E": rep(P2 / (gamma - 1))}
+    for name in I.FIELDS[5:]:
+        fields[name] = z.copy()
+    params = dict(nx=n, ny=n, nz=3, dx=1.0 / n, gamma=gamma, c_hat=0.0, c=0.0, bc=I.BC_REFLECTING, cfl=0.3,
+                  flags=I.FLAG_TAU_CORR)
+    res = _run_hydro_pair(params, fields, 20, B.QK_PATH_SWEEP)
+    ref, got = res[20]
+    for name in I.FIELDS[:5]:
+        assert np.array_equal(ref[name], got[name]), name
+    r, mx, my = got["rho"][1], got["mx"][1], got["my"][1]
+    assert np.array_equal(r, r.T) and np.array_equal(mx, my.T) and np.abs(mx).max() > 0.05
