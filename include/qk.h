@@ -86,8 +86,10 @@ int qk_init(int nx, int ny, int nz, double dx, double gamma, double c_hat, doubl
 /* Destroy a context; frees device memory the library allocated (never bound storage). */
 int qk_free(qk_ctx *ctx);
 
-/* Bytes of device memory one context needs (11 state fields, 5 RK stage fields, the
- * flattening coefficient, counters), for callers that own the allocation (torch.empty). */
+/* Bytes of device memory one context needs (11 state fields, 5 RK stage fields, the flattening
+ * coefficient, 28 scratch fields -- primitives, flux-difference accumulators, radiation
+ * reconstruction variables -- and counters), for callers that own the
+ * allocation (torch.empty). */
 size_t qk_state_bytes(int nx, int ny, int nz);
 
 /* Use caller-owned DEVICE memory (>= qk_state_bytes, 256-byte aligned) instead of

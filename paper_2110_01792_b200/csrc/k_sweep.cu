@@ -213,9 +213,12 @@ __global__ void __launch_bounds__(128) chi_dir_kernel(Geom g, double gamma, cons
                                                       const double *__restrict__ vz, double *__restrict__ cx,
                                                       double *__restrict__ cy, double *__restrict__ cz)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x - 2;
-    const int j = (int)blockIdx.y - 2, k = (int)blockIdx.z - 2;
-    if (i > g.nx + 1) return;
+    // threads are dealt out over the (nx+4) x (ny+4) cells of a plane in row-major order: no idle tail per row
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    const int w = g.nx + 4;
+    if (t >= w * (g.ny + 4)) return;
+    const int jj = t / w;
+    const int i = t - jj * w - 2, j = jj - 2, k = (int)blockIdx.y - 2;
     const int c = g.at(i, j, k), sy = g.sy, sz = g.sz;
     const double P0 = P[c];
     cx[c] = flatten_coeff_1d(gamma, P[c - 2], P[c - 1], P0, P[c + 1], P[c + 2], vx[c - 1], vx[c + 1]);
@@ -226,9 +229,11 @@ __global__ void __launch_bounds__(128) chi_dir_kernel(Geom g, double gamma, cons
 __global__ void __launch_bounds__(128) chi_min_kernel(Geom g, const double *__restrict__ cx, const double *__restrict__ cy,
                                                       const double *__restrict__ cz, double *__restrict__ chi)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x - 1;
-    const int j = (int)blockIdx.y - 1, k = (int)blockIdx.z - 1;
-    if (i > g.nx) return;
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    const int w = g.nx + 2;
+    if (t >= w * (g.ny + 2)) return;
+    const int jj = t / w;
+    const int i = t - jj * w - 1, j = jj - 1, k = (int)blockIdx.y - 1;
     const int c = g.at(i, j, k), sy = g.sy, sz = g.sz;
     double x = 1.0;      // same nesting as the oracle: min(1, min(lo, min(mid, hi))) per direction
     x = lesser(x, lesser(cx[c - 1], lesser(cx[c], cx[c + 1])));
@@ -240,7 +245,7 @@ __global__ void __launch_bounds__(128) chi_min_kernel(Geom g, const double *__re
 int launch_chi_two_pass(const Geom &g, double gamma, CHydro5 W, double *cx, double *cy, double *cz, double *chi,
                         cudaStream_t st)
 {
-    dim3 g1((g.nx + 4 + 127) / 128, g.ny + 4, g.nz + 4), g2((g.nx + 2 + 127) / 128, g.ny + 2, g.nz + 2);
+    dim3 g1(((g.nx + 4) * (g.ny + 4) + 127) / 128, g.nz + 4), g2(((g.nx + 2) * (g.ny + 2) + 127) / 128, g.nz + 2);
     chi_dir_kernel<<<g1, 128, 0, st>>>(g, gamma, W.E, W.mx, W.my, W.mz, cx, cy, cz);
     chi_min_kernel<<<g2, 128, 0, st>>>(g, cx, cy, cz, chi);
     return 2;

@@ -403,7 +403,7 @@ int qk_init(int nx, int ny, int nz, double dx, double gamma, double c_hat, doubl
     if (nx < 1 || ny < 1 || nz < 1 || !(dx > 0.0) || !(gamma > 1.0) || c_hat < 0.0 || c < 0.0) return QK_EINVAL;
     if (boundary != QK_BC_PERIODIC && boundary != QK_BC_OUTFLOW && boundary != QK_BC_REFLECTING) return QK_EINVAL;
     if ((long long)(nx + 2 * NG) * (ny + 2 * NG) * (nz + 2 * NG) > 2000000000LL) return QK_EINVAL;
-    if (ny + 2 > 65535 || nz + 2 > 65535) return QK_EINVAL;
+    if (ny + 4 > 65535 || nz + 4 > 65535) return QK_EINVAL;
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return QK_ECUDA; }
     qk_ctx *x = new (std::nothrow) qk_ctx();
