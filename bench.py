@@ -41,6 +41,7 @@ OPS_HYDRO_STAGE = 1240.0    # S3 12 + S4 62 + S5 810 + S6 318 + S7 38
 OPS_HYDRO_SWEEP = 388.0     # one direction of one stage: S5 270 + S6 106 + its share of S7 12
 OPS_RAD_STAGE = 1080.0      # S8 640 + S9 402 + S10 38
 OPS_RAD_SWEEP = 357.0       # one direction: S8 214 + S9 134 + its share of S10 9
+HYDRO_WORKLOAD = "config2"  # --workload sedov: the paper's own hydro benchmark problem, context only
 SCHEME_FLAGS = 0            # --plm / --eddington: scheme variants; the headline run uses PPM + Levermore
 BYTES_EXCHANGE = 224.0      # 11 reads + 8 writes (eq 26-43) + the 9 reconstruction variables it leaves for the next stage
 # dram__bytes_read.sum + dram__bytes_write.sum per launch at 256^3 from the ncu --set full capture summarised in
@@ -237,7 +238,10 @@ def time_steps_e2e(torch, ctx, kind, nsteps, host_in, host_out, barrier, ex=None
 def run_workload(torch, B, I, kind, n, steps, warmup, rank, world, barrier, allmax, sampler=None, path=None,
                  decompose=False):
     t0 = time.time()
-    params, fields = (I.config2(n=n, seed=1002 + rank) if kind == "hydro" else I.config4(n=n, seed=1004 + rank))
+    if kind == "hydro":
+        params, fields = I.sedov(n=n) if HYDRO_WORKLOAD == "sedov" else I.config2(n=n, seed=1002 + rank)
+    else:
+        params, fields = I.config4(n=n, seed=1004 + rank)
     params["flags"] |= SCHEME_FLAGS
     log("[rank %d] %s %d^3 inputs generated in %.1f s" % (rank, kind, n, time.time() - t0))
     nf = 5 if kind == "hydro" else 9
@@ -382,8 +386,11 @@ def run_ours(args):
         "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": hyd["ms"] / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "BASELINE.json configs[1]: pure hydro %d^3, periodic, gamma=5/3, log-normal density, "
-                               "k^-2 velocity field at rms Mach 2, CFL 0.3, qk_cfl_dt + qk_hydro_step per step" % n,
+        "config": {"workload": ("BASELINE.json configs[1]: pure hydro %d^3, periodic, gamma=5/3, log-normal density, "
+                                "k^-2 velocity field at rms Mach 2, CFL 0.3, qk_cfl_dt + qk_hydro_step per step" % n)
+                               if HYDRO_WORKLOAD == "config2" else
+                               ("Sedov blast %d^3 on [-1,1]^3, periodic, gamma=5/3, CFL 0.25 (PAPER.md:572), "
+                                "qk_cfl_dt + qk_hydro_step per step" % n),
                    "scheme": ("PLM" if SCHEME_FLAGS & 8 else "PPM") + (" + Eddington closure" if SCHEME_FLAGS & 16 else " + Levermore closure"),
                    "cells": cells, "l2": "inputs larger than L2 (5 x %.0f MB per stage)" % (cells * 8 / 1e6),
                    "parallelism": hyd.get("parallelism", "1 box on 1 GPU") if world > 1 else "1 box on 1 GPU"},
@@ -443,13 +450,16 @@ def main():
     ap.add_argument("--path", default="sweep", choices=["fused", "unfused", "sweep"], help="stage kernel family")
     ap.add_argument("--replicas", action="store_true",
                     help="N>1: independent boxes per GPU instead of one z-slab-decomposed global box")
+    ap.add_argument("--workload", default="config2", choices=["config2", "sedov"],
+                    help="hydro workload: BASELINE configs[1] (default, the metric) or the paper's Sedov blast (CFL 0.25)")
     ap.add_argument("--plm", action="store_true", help="PLM + MC limiter instead of PPM (PAPER.md:164)")
     ap.add_argument("--eddington", action="store_true", help="Eddington approximation instead of the Levermore closure")
     ap.add_argument("--no-rhd", action="store_true")
     ap.add_argument("--no-hydro", action="store_true", help="profiling aid: run only the RHD workload")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
-    global SCHEME_FLAGS
+    global SCHEME_FLAGS, HYDRO_WORKLOAD
+    HYDRO_WORKLOAD = args.workload
     SCHEME_FLAGS = (8 if args.plm else 0) | (16 if args.eddington else 0)
     if args.impl == "reference":
         run_reference(args)

@@ -10,7 +10,10 @@
 
 namespace qk {
 
-__global__ void __launch_bounds__(128) exchange_kernel(Geom g, ExchangeConsts kc, double dt, const double *__restrict__ rho,
+#ifndef QK_EX_MINB
+#define QK_EX_MINB 6     // <= 85 registers: 1.09 -> 1.04 ms at 256^3; 8 spills into the Newton loop (1.45 ms)
+#endif
+__global__ void __launch_bounds__(128, QK_EX_MINB) exchange_kernel(Geom g, ExchangeConsts kc, double dt, const double *__restrict__ rho,
                                                        double *__restrict__ mx, double *__restrict__ my,
                                                        double *__restrict__ mz, double *__restrict__ E,
                                                        double *__restrict__ Er, double *__restrict__ Fx,

@@ -181,6 +181,29 @@ def test_hydro_sedov_small_bitwise():
     print("sedov mismatching cells:", P.count_mismatch(*res[8], I.FIELDS[:5]))
 
 
+def test_side_stream_and_two_contexts():
+    """qk_set_stream: all work of a context goes to the stream it was given (a non-default torch stream here),
+    and two contexts with different boxes advance independently (no global state in the library)."""
+    import torch
+    pa, fa = I.ragged_hydro(seed=3)
+    pb, fb = I.ragged_hydro(shape=(12, 9, 40), seed=4, bc=B.QK_BC_OUTFLOW)
+    ga, gb = P.make_oracle(pa, fa), P.make_oracle(pb, fb)
+    side = torch.cuda.Stream()
+    with P.make_gpu(pa, fa) as ca, P.make_gpu(pb, fb) as cb:
+        ca.qk_set_stream(side.cuda_stream)
+        with torch.cuda.stream(side):
+            for _ in range(3):
+                dta, dtb = ga.cfl_dt(), gb.cfl_dt()
+                assert ca.qk_cfl_dt() == dta and cb.qk_cfl_dt() == dtb
+                ca.qk_hydro_step(dta)           # interleaved launches on two streams
+                cb.qk_hydro_step(dtb)
+                assert ga.hydro_step(dta) == 0 and gb.hydro_step(dtb) == 0
+        side.synchronize()
+        P.assert_parity(ga.get_all(I.FIELDS[:5]), ca.get_all(I.FIELDS[:5]), P.TOL_ONE_STEP, P.HYDRO, "side stream")
+        P.assert_parity(gb.get_all(I.FIELDS[:5]), cb.get_all(I.FIELDS[:5]), P.TOL_ONE_STEP, P.HYDRO, "second context")
+    ga.close(), gb.close()
+
+
 def test_hydro_uniform_state_is_invariant():
     n = 16
     shape = (n, n, n)
