@@ -103,6 +103,13 @@ int qk_set_stream(qk_ctx *ctx, void *cuda_stream);
  * T = (gamma-1) E_g / (rho k_B/(mu m_H)) (X2). */
 int qk_set_constants(qk_ctx *ctx, double a_rad, double kB_over_mu_mH);
 
+/* Equation of state of the gas in the EXCHANGE step: QK_EOS_IDEAL (default; T = (gamma-1) E_g / (rho k_B/(mu m_H)))
+ * or QK_EOS_ALPHA_T3, E_g = alpha T^4 / 4 with volumetric heat capacity C_v = alpha T^3 (eq 55, PAPER.md:424-427;
+ * the Marshak, Su-Olson and energy-exchange tests, where the matter is static).  The hydro step always uses the
+ * ideal gas. */
+enum { QK_EOS_IDEAL = 0, QK_EOS_ALPHA_T3 = 1 };
+int qk_set_eos(qk_ctx *ctx, int eos, double alpha);
+
 /* CFL number C0/D of eq 21, Newton tolerance and iteration cap,
  * N_sub,max and QK_FLAG_* bits. */
 int qk_set_params(qk_ctx *ctx, double cfl, double newton_tol, int newton_maxit, int nsub_max,

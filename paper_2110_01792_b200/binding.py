@@ -29,7 +29,7 @@ EXPORTS = [
     "qk_cfl_dt", "qk_hydro_step", "qk_rad_transport", "qk_exchange", "qk_rad_step", "qk_rhd_step",
     "qk_nsub_for", "qk_last_info", "qk_launch_count", "qk_set_path", "qk_set_profiling",
     "qk_kernel_class_count", "qk_kernel_class_name", "qk_kernel_times", "qk_version", "qk_fp64_probe",
-    "qk_selftest_divsqrt", "qk_set_halo_exchange", "qk_halo_doubles", "qk_halo_pack", "qk_halo_unpack",
+    "qk_selftest_divsqrt", "qk_set_eos", "qk_set_halo_exchange", "qk_halo_doubles", "qk_halo_pack", "qk_halo_unpack",
 ]
 
 
@@ -40,6 +40,7 @@ class qk_info(C.Structure):
 
 
 QK_FACE_ZLO, QK_FACE_ZHI = 1, 2
+QK_EOS_IDEAL, QK_EOS_ALPHA_T3 = 0, 1
 HALO_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_int)
 
 
@@ -68,6 +69,7 @@ def lib():
         "qk_set_stream": (i, [p, p]),
         "qk_set_constants": (i, [p, d, d]),
         "qk_set_params": (i, [p, d, d, i, i, u]),
+        "qk_set_eos": (i, [p, i, d]),
         "qk_set_state": (i, [p, i, p]),
         "qk_get_state": (i, [p, i, p]),
         "qk_set_raw": (i, [p, i, p]),
@@ -187,6 +189,9 @@ class Context:
 
     def qk_set_params(self, cfl=0.3, newton_tol=1e-10, newton_maxit=400, nsub_max=10, flags=QK_FLAG_TAU_CORR):
         _check(self.L.qk_set_params(self.h, cfl, newton_tol, newton_maxit, nsub_max, flags), "qk_set_params")
+
+    def qk_set_eos(self, eos, alpha=0.0):
+        _check(self.L.qk_set_eos(self.h, eos, alpha), "qk_set_eos")
 
     def qk_set_path(self, path):
         _check(self.L.qk_set_path(self.h, path), "qk_set_path")

@@ -79,6 +79,7 @@ int launch_exchange(const Geom &g, const PhysConsts &pc, double dt, const double
     ExchangeConsts kc;
     kc.c = pc.c; kc.c_hat = pc.c_hat; kc.a_rad = pc.a_rad; kc.kB_mu = pc.kB_mu; kc.gamma = pc.gamma;
     kc.tol = pc.newton_tol; kc.maxit = pc.newton_maxit;
+    kc.alpha = pc.eos_alpha; kc.eos_alpha_t3 = pc.eos_alpha > 0.0;
     kc.literal_stop = (pc.flags & QK_FLAG_NEWTON_LITERAL) != 0;
     kc.static_matter = (pc.flags & QK_FLAG_STATIC_MATTER) != 0;
     dim3 grid((g.nx + 127) / 128, g.ny, g.nz);

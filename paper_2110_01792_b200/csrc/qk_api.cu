@@ -410,7 +410,7 @@ int qk_init(int nx, int ny, int nz, double dx, double gamma, double c_hat, doubl
     if (!x) return QK_ENOMEM;
     x->g = make_geom(nx, ny, nz);
     x->pc.dx = dx; x->pc.gamma = gamma; x->pc.c_hat = c_hat; x->pc.c = c;
-    x->pc.a_rad = 1.0; x->pc.kB_mu = 1.0; x->pc.cfl = 0.3; x->pc.newton_tol = 1e-10;
+    x->pc.a_rad = 1.0; x->pc.kB_mu = 1.0; x->pc.eos_alpha = 0.0; x->pc.cfl = 0.3; x->pc.newton_tol = 1e-10;
     x->pc.newton_maxit = 400; x->pc.nsub_max = 10; x->pc.flags = QK_FLAG_TAU_CORR; x->pc.bc = boundary;
     x->stream = nullptr; x->device = dev; x->base = nullptr; x->bytes = 0; x->owns = false; x->ready = false;
     x->path = QK_PATH_SWEEP; x->w_cur = 0; x->s_cur = 0; x->w_valid = false; x->s_valid = false; x->smax_valid = false;
@@ -458,6 +458,13 @@ int qk_set_constants(qk_ctx *c, double a_rad, double kB_over_mu_mH)
 {
     if (!c || !(a_rad >= 0.0) || !(kB_over_mu_mH > 0.0)) return QK_EINVAL;
     c->pc.a_rad = a_rad; c->pc.kB_mu = kB_over_mu_mH;
+    return QK_OK;
+}
+
+int qk_set_eos(qk_ctx *c, int eos, double alpha)
+{
+    if (!c || (eos != QK_EOS_IDEAL && eos != QK_EOS_ALPHA_T3) || (eos == QK_EOS_ALPHA_T3 && !(alpha > 0.0))) return QK_EINVAL;
+    c->pc.eos_alpha = eos == QK_EOS_ALPHA_T3 ? alpha : 0.0;
     return QK_OK;
 }
 

@@ -59,6 +59,7 @@ enum KClass { K_FILL = 0, K_CFL, K_PRIM, K_FLATTEN, K_HYDRO_FLUX, K_HYDRO_UPDATE
 
 struct PhysConsts {
     double dx, gamma, c_hat, c, a_rad, kB_mu, cfl, newton_tol;
+    double eos_alpha;      // > 0: E_g = alpha T^4 / 4 in the exchange (eq 55); 0: ideal gas
     int newton_maxit, nsub_max;
     unsigned flags;
     int bc;

@@ -265,6 +265,8 @@ QK_HD Rad4 rad_hll_flux(double c, double c_hat, double EL, double fxL, double fy
 
 struct ExchangeConsts {
     double c, c_hat, a_rad, kB_mu, gamma, tol;
+    double alpha;          // eos_alpha_t3: E_g = alpha T^4 / 4, C_v = alpha T^3 (eq 55)
+    bool eos_alpha_t3;
     int maxit;
     bool literal_stop, static_matter;
 };
@@ -282,12 +284,19 @@ QK_HD int exchange_cell(const ExchangeConsts &k, double dt, double rho, double &
     const double Er_old = Er;
     const double Etot = Eg_old + c_ratio * Er_old;              // eq 38 with S = 0
     const double coef = dt * rho * kappaP * k.c_hat;            // dt rho kappa_P c_hat (X1)
-    const double Cv = rho * k.kB_mu / (k.gamma - 1.0);          // volumetric heat capacity (X2)
+    const double Cv_ideal = rho * k.kB_mu / (k.gamma - 1.0);    // volumetric heat capacity (X2)
     double Eg = Eg_old, Erad = Er_old;
     int it = 0;
     bool finished = false;
     while (it < k.maxit) {
-        const double T = Eg / Cv;
+        double T, Cv;
+        if (k.eos_alpha_t3) {                                             // eq 55
+            T = sqrt(sqrt(4.0 * Eg / k.alpha));
+            Cv = k.alpha * (T * T * T);
+        } else {
+            Cv = Cv_ideal;
+            T = Eg / Cv;
+        }
         const double T2 = T * T;
         const double T4 = T2 * T2;
         const double R = coef * (k.a_rad * T4 - Erad);                    // eq 28 (X1)
