@@ -133,6 +133,21 @@ __device__ __forceinline__ void plm_states(Q q, double lo[NV], double hi[NV])
     }
 }
 
+// Marching sweeps: the raw interface value at the high face of one cell is the raw interface value at the low
+// face of the next (the same expression of eq 22 on the same four cells), so it is carried in `ifc` instead of
+// being evaluated twice; q(v, 0) is then never read.  Same values as ppm_cell / rad_ppm_cell.
+template <int BL, int NV, typename Q>
+__device__ __forceinline__ void ppm_states_carry(Q q, double ifc[NV], double lo[NV], double hi[NV])
+{
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+        const double b = q(v, 1), c = q(v, 2), d = q(v, 3), e = q(v, 4);
+        const double hi_raw = ppm_interface(b, c, d, e);
+        ppm_limit_t<BL != 0>(ifc[v], hi_raw, b, c, d, lo[v], hi[v]);
+        ifc[v] = hi_raw;
+    }
+}
+
 // flattened PPM face states of all five primitives of one cell; q(v, m) = value of variable v at
 // stencil offset m-2
 template <int BL = 0, typename Q>

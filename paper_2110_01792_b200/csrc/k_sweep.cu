@@ -49,7 +49,8 @@ struct HydroPhT {
     static constexpr int NV = 5;
     static constexpr bool COUNTS = false;
     // select-only PPM limiter (same values): measured faster in the x sweep, slower in the marching sweeps
-    static constexpr int BL_X = QK_BLX_H, BL_MARCH = QK_BLM_H;   // 0 branches, 1 selects, 2 selects in lockstep
+    static constexpr int BL_X = QK_BLX_H, BL_MARCH = QK_BLM_H;
+    static constexpr bool CARRY = true;    // marching sweeps carry the raw interface value (measured: -1.5 %)   // 0 branches, 1 selects, 2 selects in lockstep
     const double *w[5];        // rho, vx, vy, vz, P (ghost cells included)
     const double *chi;         // flattening coefficient of the cells -1..n
     double gamma;
@@ -73,6 +74,20 @@ struct HydroPhT {
             }
         } else {
             ppm_cell<BL>(q, x, lo, hi);
+        }
+        return 0;
+    }
+    template <int BL, class Q>
+    __device__ __forceinline__ int states_carry(Q q, double x, double ifc[5], double lo[5], double hi[5]) const
+    {
+        if (RECON == 1) return states<BL>(q, x, lo, hi);
+        double l[5], h[5];
+        ppm_states_carry<BL, 5>(q, ifc, l, h);
+#pragma unroll
+        for (int v = 0; v < 5; ++v) {
+            const double c = q(v, 2);
+            lo[v] = c + x * (l[v] - c);         // flatten toward the cell average
+            hi[v] = c + x * (h[v] - c);
         }
         return 0;
     }
@@ -132,6 +147,7 @@ struct RadPhT {
     static constexpr int NV = 4;
     static constexpr bool COUNTS = true;
     static constexpr int BL_X = QK_BLX_R, BL_MARCH = QK_BLM_R;
+    static constexpr bool CARRY = false;   // measured slower with the select-only limiter (+1.5 %)
     const double *s[4];        // E_r, fx, fy, fz
     const double *rho, *kR;
     double c, c_hat, dx;
@@ -154,6 +170,26 @@ struct RadPhT {
     {
         if (RECON == 0) return rad_ppm_cell<BL>(q, lo, hi);
         plm_states<4>(q, lo, hi);
+        int nfall = 0;      // first-order fallback per face state, as in rad_ppm_cell
+        double f2 = (lo[1] * lo[1] + lo[2] * lo[2]) + lo[3] * lo[3];
+        if (f2 > 1.0 || !(lo[0] > 0.0)) {
+#pragma unroll
+            for (int v = 0; v < 4; ++v) lo[v] = q(v, 2);
+            ++nfall;
+        }
+        f2 = (hi[1] * hi[1] + hi[2] * hi[2]) + hi[3] * hi[3];
+        if (f2 > 1.0 || !(hi[0] > 0.0)) {
+#pragma unroll
+            for (int v = 0; v < 4; ++v) hi[v] = q(v, 2);
+            ++nfall;
+        }
+        return nfall;
+    }
+    template <int BL, class Q>
+    __device__ __forceinline__ int states_carry(Q q, double x, double ifc[4], double lo[4], double hi[4]) const
+    {
+        if (RECON == 1) return states<BL>(q, x, lo, hi);
+        ppm_states_carry<BL, 4>(q, ifc, lo, hi);
         int nfall = 0;      // first-order fallback per face state, as in rad_ppm_cell
         double f2 = (lo[1] * lo[1] + lo[2] * lo[2]) + lo[3] * lo[3];
         if (f2 > 1.0 || !(lo[0] > 0.0)) {

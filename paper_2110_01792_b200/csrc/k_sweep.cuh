@@ -182,9 +182,13 @@ __global__ void __launch_bounds__(SW_NT, MODE == 2 ? QK_SW_MINB2 : QK_SW_MINB1) 
 #pragma unroll
     for (int v = 0; v < SW_NR; ++v) pend[v] = ph.ld(v, base + (m0 + 1) * s);
     double aux_next = ph.aux(base + (m0 - 1) * s);
-    double hiP[NV], Flo[NV];
+    double hiP[NV], Flo[NV], ifc[NV];
 #pragma unroll
-    for (int v = 0; v < NV; ++v) { hiP[v] = 0.0; Flo[v] = 0.0; }
+    for (int v = 0; v < NV; ++v) {
+        hiP[v] = 0.0; Flo[v] = 0.0;
+        // raw eq 22 interface at the low face of the first cell reconstructed (cells m0-3..m0 are in r0..r3)
+        ifc[v] = ppm_interface(ring[r0 + v * SW_NT], ring[r1 + v * SW_NT], ring[r2 + v * SW_NT], ring[r3 + v * SW_NT]);
+    }
     int nfall = 0, nguard = 0;
 
     for (int m = m0 - 2; m < m1; ++m) {
@@ -214,7 +218,9 @@ __global__ void __launch_bounds__(SW_NT, MODE == 2 ? QK_SW_MINB2 : QK_SW_MINB1) 
         double lo[NV], hi[NV], Fhi[NV];
         {
             const int rr[5] = {r0, r1, r2, r3, r4};
-            const int nf = ph.template states<PH::BL_MARCH>([&](int v, int q) { return ring[rr[q] + v * SW_NT]; }, aux, lo, hi);
+            const auto win = [&](int v, int q) { return ring[rr[q] + v * SW_NT]; };
+            const int nf = PH::CARRY ? ph.template states_carry<PH::BL_MARCH>(win, aux, ifc, lo, hi)
+                                     : ph.template states<PH::BL_MARCH>(win, aux, lo, hi);
             const int mm = m + 1;
             if (PH::COUNTS && active && ((mm >= m0 && mm < m1) || mm == -1 || mm == n_m)) nfall += nf;
         }

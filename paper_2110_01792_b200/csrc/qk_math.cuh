@@ -58,12 +58,16 @@ QK_HD double mc_slope(double qW, double qC, double qE)
 // eq 22 interface values with mirror-symmetric brackets, three-cell clamp
 // (H3), then the parabola check: extremum -> MC-limited line (H4), one-sided
 // overshoot -> CW84 correction (H5).  qlo = state at j-1/2, qhi = state at j+1/2.
-template <bool BRANCHLESS>
-QK_HD void ppm_face_states_t(double a, double b, double c, double d, double e, double &qlo, double &qhi)
+// eq 22 interface value between the cells m and p, with their outer neighbours mm (beyond m) and pp (beyond p)
+QK_HD double ppm_interface(double mm, double m, double p, double pp)
 {
-    const double w7 = 7.0 / 12.0, w1 = 1.0 / 12.0;
-    double lo_face = w7 * (b + c) - w1 * (d + a);
-    double hi_face = w7 * (c + d) - w1 * (e + b);
+    return (7.0 / 12.0) * (m + p) - (1.0 / 12.0) * (pp + mm);
+}
+
+// Limiting steps of PPM for one cell (b, c, d) given the two raw interface values of eq 22.
+template <bool BRANCHLESS>
+QK_HD void ppm_limit_t(double lo_face, double hi_face, double b, double c, double d, double &qlo, double &qhi)
+{
     const double floor3 = lesser(b, lesser(c, d));
     const double ceil3 = greater(b, greater(c, d));
     lo_face = lesser(greater(lo_face, floor3), ceil3);
@@ -94,6 +98,12 @@ QK_HD void ppm_face_states_t(double a, double b, double c, double d, double e, d
     }
     qlo = lo_face;
     qhi = hi_face;
+}
+
+template <bool BRANCHLESS>
+QK_HD void ppm_face_states_t(double a, double b, double c, double d, double e, double &qlo, double &qhi)
+{
+    ppm_limit_t<BRANCHLESS>(ppm_interface(a, b, c, d), ppm_interface(b, c, d, e), b, c, d, qlo, qhi);
 }
 
 QK_HD void ppm_face_states(double a, double b, double c, double d, double e, double &qlo, double &qhi)
