@@ -42,6 +42,7 @@ OPS_HYDRO_SWEEP = 388.0     # one direction of one stage: S5 270 + S6 106 + its 
 OPS_RAD_STAGE = 1080.0      # S8 640 + S9 402 + S10 38
 OPS_RAD_SWEEP = 357.0       # one direction: S8 214 + S9 134 + its share of S10 9
 HYDRO_WORKLOAD = "config2"  # --workload sedov: the paper's own hydro benchmark problem, context only
+CHAT_RATIO = 0.01           # --chat-ratio: c_hat/c of the RHD workload (0.01 = BASELINE configs[3]; 0.5 gives N_sub = 10)
 SCHEME_FLAGS = 0            # --plm / --eddington: scheme variants; the headline run uses PPM + Levermore
 BYTES_EXCHANGE = 224.0      # 11 reads + 8 writes (eq 26-43) + the 9 reconstruction variables it leaves for the next stage
 # dram__bytes_read.sum + dram__bytes_write.sum per launch at 256^3 from the ncu --set full capture summarised in
@@ -241,7 +242,7 @@ def run_workload(torch, B, I, kind, n, steps, warmup, rank, world, barrier, allm
     if kind == "hydro":
         params, fields = I.sedov(n=n) if HYDRO_WORKLOAD == "sedov" else I.config2(n=n, seed=1002 + rank)
     else:
-        params, fields = I.config4(n=n, seed=1004 + rank)
+        params, fields = I.config4(n=n, seed=1004 + rank, chat_ratio=CHAT_RATIO)
     params["flags"] |= SCHEME_FLAGS
     log("[rank %d] %s %d^3 inputs generated in %.1f s" % (rank, kind, n, time.time() - t0))
     nf = 5 if kind == "hydro" else 9
@@ -416,8 +417,8 @@ def run_ours(args):
         line["rhd"] = {
             "metric": "rhd_cell_updates_per_s", "value": rhd["value"], "unit": UNIT, "steps": rhd["steps"],
             "ms_per_step": rhd["ms"] / rhd["steps"], "nsub": rhd["info"]["nsub"],
-            "config": {"workload": "BASELINE.json configs[3]: coupled RHD %d^3, periodic, c_hat/c=0.01, "
-                                   "qk_cfl_dt + qk_rhd_step per step" % n},
+            "config": {"workload": "BASELINE.json configs[3]: coupled RHD %d^3, periodic, c_hat/c=%g, "
+                                   "qk_cfl_dt + qk_rhd_step per step" % (n, CHAT_RATIO)},
             "e2e": rhd["e2e"], "gpu_launches": rhd["launches"],
             "roofline_rad": rroof, "roofline_exchange": exroof,
             "kernel_ms": {k: {"total_ms": v[0], "groups": v[1]} for k, v in rhd["kernel_ms"].items()},
@@ -452,13 +453,17 @@ def main():
                     help="N>1: independent boxes per GPU instead of one z-slab-decomposed global box")
     ap.add_argument("--workload", default="config2", choices=["config2", "sedov"],
                     help="hydro workload: BASELINE configs[1] (default, the metric) or the paper's Sedov blast (CFL 0.25)")
+    ap.add_argument("--chat-ratio", type=float, default=0.01,
+                    help="c_hat/c of the RHD workload; 0.5 makes every step take N_sub = N_sub,max = 10 radiation "
+                         "substeps like the paper's RHD benchmark (PAPER.md:604)")
     ap.add_argument("--plm", action="store_true", help="PLM + MC limiter instead of PPM (PAPER.md:164)")
     ap.add_argument("--eddington", action="store_true", help="Eddington approximation instead of the Levermore closure")
     ap.add_argument("--no-rhd", action="store_true")
     ap.add_argument("--no-hydro", action="store_true", help="profiling aid: run only the RHD workload")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
-    global SCHEME_FLAGS, HYDRO_WORKLOAD
+    global SCHEME_FLAGS, HYDRO_WORKLOAD, CHAT_RATIO
+    CHAT_RATIO = args.chat_ratio
     HYDRO_WORKLOAD = args.workload
     SCHEME_FLAGS = (8 if args.plm else 0) | (16 if args.eddington else 0)
     if args.impl == "reference":

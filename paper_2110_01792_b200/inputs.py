@@ -118,7 +118,7 @@ def config3(n=128, seed=1003, shape=None):
     return params, _fill_missing(fields, shape)
 
 
-def config4(n=256, seed=1004, kmax=16, shape=None):
+def config4(n=256, seed=1004, kmax=16, shape=None, chat_ratio=0.01):
     """BASELINE.json configs[3]/[4]: coupled RHD, periodic, c/c_s ~ 100, c_hat/c = 0.01."""
     shape = shape or (n, n, n)
     gamma = 5.0 / 3.0
@@ -126,7 +126,7 @@ def config4(n=256, seed=1004, kmax=16, shape=None):
     dx = 1.0 / shape[2]
     kmax = min(kmax, max(1, min(shape) // 4))
     c = 100.0 * np.sqrt(gamma)
-    c_hat = 0.01 * c
+    c_hat = chat_ratio * c      # BASELINE configs[3]: c_hat/c = 0.01 (N_sub = 1); larger ratios force subcycling
     rho = np.exp(0.5 * spectral_field(rng, shape, kmax=kmax) - 0.125)
     tf = spectral_field(rng, shape, kmax=kmax)
     ranks = np.empty(tf.size, dtype=np.float64)
