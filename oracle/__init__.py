@@ -19,7 +19,7 @@ _SRCS = ["grid.c", "hydro.c", "radiation.c", "exchange.c"]
 _LIB = os.path.join(_HERE, "libqk_oracle.so")
 
 NG = 4
-FIELDS = ["rho", "mx", "my", "mz", "E", "Er", "Fx", "Fy", "Fz", "kappaP", "kappaR"]
+FIELDS = ["rho", "mx", "my", "mz", "E", "Er", "Fx", "Fy", "Fz", "kappaP", "kappaR", "src"]
 BC_PERIODIC, BC_OUTFLOW, BC_REFLECTING = 0, 1, 2
 FLAG_TAU_CORR, FLAG_STATIC_MATTER, FLAG_NEWTON_LITERAL = 1, 2, 4
 FLAG_PLM, FLAG_EDDINGTON = 8, 16

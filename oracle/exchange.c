@@ -97,6 +97,7 @@ int orc_exchange(orc_grid *g, double dt)
                 double F[3] = { g->f[ORC_FX][cidx], g->f[ORC_FY][cidx], g->f[ORC_FZ][cidx] };
                 double E = g->f[ORC_E][cidx], Er = g->f[ORC_ER][cidx];
                 int it = 0;
+                g->S_src = dt * g->f[ORC_SRC][cidx];            /* energy added during the substep (X13) */
                 int r = orc_exchange_cell(g, dt, g->f[ORC_RHO][cidx], m, &E, &Er, F,
                                           g->f[ORC_KP][cidx], g->f[ORC_KR][cidx], &it);
                 if (r == 4) ++fail;
@@ -106,6 +107,7 @@ int orc_exchange(orc_grid *g, double dt)
                 g->f[ORC_FX][cidx] = F[0]; g->f[ORC_FY][cidx] = F[1]; g->f[ORC_FZ][cidx] = F[2];
                 g->f[ORC_E][cidx] = E; g->f[ORC_ER][cidx] = Er;
             }
+    g->S_src = 0.0;
     g->newton_fail_cells = fail; g->newton_total_iters = tot; g->newton_max_iters = mx;
     g->bad_state_cells = bad;
     return fail ? 4 : (bad ? 5 : 0);

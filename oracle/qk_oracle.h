@@ -34,10 +34,11 @@ extern "C" {
 #endif
 
 #define ORC_NG 4          /* ghost zones per side (BASELINE.json config 1) */
-#define ORC_NFIELDS 11    /* rho mx my mz E Er Fx Fy Fz kappaP kappaR      */
+#define ORC_NFIELDS 12    /* rho mx my mz E Er Fx Fy Fz kappaP kappaR src  */
 
 enum { ORC_RHO = 0, ORC_MX, ORC_MY, ORC_MZ, ORC_E, ORC_ER, ORC_FX, ORC_FY, ORC_FZ,
-       ORC_KP, ORC_KR };
+       ORC_KP, ORC_KR,
+       ORC_SRC };   /* radiation energy source rate per cell: S of eq 27 is dt * src (reading X13) */
 enum { ORC_BC_PERIODIC = 0, ORC_BC_OUTFLOW = 1,
        ORC_BC_REFLECTING = 2 };  /* solid wall: mirror image, normal momentum / flux component negated */
 enum { ORC_FLAG_TAU_CORR = 1, ORC_FLAG_STATIC_MATTER = 2, ORC_FLAG_NEWTON_LITERAL = 4,
@@ -55,7 +56,8 @@ typedef struct orc_grid {
     int newton_maxit, nsub_max;
     unsigned flags;
     int eos; double alpha;          /* ORC_EOS_ALPHA_T3: E_g = alpha T^4 / 4           */
-    double S_src;                   /* uniform source S of eq 27 (0 in every config)   */
+    double S_src;                   /* S of eq 27 for the cell orc_exchange_cell is called on; orc_exchange sets it
+                                       to dt * f[ORC_SRC][cell] (0 in every BASELINE config)                  */
     double *f[ORC_NFIELDS];         /* (nz+8)(ny+8)(nx+8) each, x fastest              */
     /* diagnostics of the last call */
     int last_nsub;

@@ -165,3 +165,35 @@ def test_rhd_conservation_3d():
     assert info["newton_fail_cells"] == 0 and info["nsub"] >= 1
     for a, b, s in zip(t0, totals(), scale):
         assert abs(a - b) < 1e-12 * s, (a, b)
+
+
+def test_source_term_of_eq27():
+    """PAPER.md:215 (eq 27, 38): S adds radiation energy during the substep; reading X13: S = dt * rate(cell).
+    Transparent gas (kappa_P = 0): E_r grows by exactly dt*rate per step and the gas is untouched.  Opaque gas:
+    eq 26 + (c/c_hat) eq 27 give  Delta(E_g + (c/c_hat) E_r) = (c/c_hat) S  per step, whatever the Newton path."""
+    c, ch = 10.0, 2.0
+    n = 3
+    shape = (n, n, n)
+    rng = np.random.default_rng(4)
+    rate = rng.uniform(0.5, 2.0, shape)
+    for kappa in (0.0, 5.0):
+        g = O.Grid(n, n, n, 1.0, 5.0 / 3.0, c_hat=ch, c=c)
+        g.set_params(flags=O.FLAG_STATIC_MATTER)
+        rho = rng.uniform(0.5, 2.0, shape)
+        E0 = rng.uniform(1.0, 2.0, shape)
+        Er0 = rng.uniform(0.5, 1.5, shape)
+        for name, a in (("rho", rho), ("E", E0), ("Er", Er0), ("kappaP", np.full(shape, kappa)),
+                        ("kappaR", np.full(shape, kappa)), ("src", rate)):
+            g.set_state(O.FIELDS.index(name), a)
+        dt, nsteps = 0.01, 7
+        for s in range(1, nsteps + 1):
+            assert g.exchange(dt) == 0
+            E, Er = g.get_state(4), g.get_state(5)
+            budget = (E + (c / ch) * Er) - (E0 + (c / ch) * Er0)
+            assert np.abs(budget - (c / ch) * s * dt * rate).max() < 1e-13 * (c / ch) * 10
+            if kappa == 0.0:
+                assert np.array_equal(E, E0)
+                assert np.abs(Er - (Er0 + s * dt * rate)).max() < 1e-14
+        if kappa > 0.0:
+            assert np.abs(g.get_state(4) - E0).max() > 1e-3      # the gas does take up part of the injected energy
+        g.close()
