@@ -42,6 +42,8 @@ enum { QK_BC_PERIODIC = 0,   /* PAPER.md:293, 572 */
  * (E_r, F_r) (eq 11-12), Planck- and Rosseland-type opacities per cell
  * (kappa_E~kappa_P, kappa_F~kappa_R), static during a step. */
 enum { QK_RHO = 0, QK_MX, QK_MY, QK_MZ, QK_E, QK_ER, QK_FX, QK_FY, QK_FZ, QK_KAPPA_P, QK_KAPPA_R,
+       QK_SRC,      /* radiation energy source rate per cell (e.g. stellar sources): the S of eq 27 / 38 is dt * src
+                       (reading X13); zero unless set; read by the exchange step only */
        QK_NFIELDS };
 
 enum { QK_FLAG_TAU_CORR = 1,        /* guarded optical-depth correction of the E_r HLL flux (R6) */
@@ -86,7 +88,7 @@ int qk_init(int nx, int ny, int nz, double dx, double gamma, double c_hat, doubl
 /* Destroy a context; frees device memory the library allocated (never bound storage). */
 int qk_free(qk_ctx *ctx);
 
-/* Bytes of device memory one context needs (11 state fields, 5 RK stage fields, the flattening
+/* Bytes of device memory one context needs (12 state fields, 5 RK stage fields, the flattening
  * coefficient, 28 scratch fields -- primitives, flux-difference accumulators, radiation
  * reconstruction variables -- and counters), for callers that own the
  * allocation (torch.empty). */

@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libqk.so")
 
 NG = 4
-FIELDS = ["rho", "mx", "my", "mz", "E", "Er", "Fx", "Fy", "Fz", "kappaP", "kappaR"]
+FIELDS = ["rho", "mx", "my", "mz", "E", "Er", "Fx", "Fy", "Fz", "kappaP", "kappaR", "src"]
 QK_OK, QK_EINVAL, QK_ENOMEM, QK_ECUDA, QK_ENEWTON, QK_ESTATE = range(6)
 QK_BC_PERIODIC, QK_BC_OUTFLOW, QK_BC_REFLECTING = 0, 1, 2
 QK_FLAG_TAU_CORR, QK_FLAG_STATIC_MATTER, QK_FLAG_NEWTON_LITERAL = 1, 2, 4

@@ -19,7 +19,7 @@ __global__ void __launch_bounds__(128, QK_EX_MINB) exchange_kernel(Geom g, Excha
                                                        double *__restrict__ Er, double *__restrict__ Fx,
                                                        double *__restrict__ Fy, double *__restrict__ Fz,
                                                        const double *__restrict__ kP, const double *__restrict__ kR,
-                                                       Hydro5 Wout, Rad4p Sout, Counters *ctr, StateCache *cache)
+                                                       const double *__restrict__ src, Hydro5 Wout, Rad4p Sout, Counters *ctr, StateCache *cache)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y, k = blockIdx.z;
@@ -30,7 +30,8 @@ __global__ void __launch_bounds__(128, QK_EX_MINB) exchange_kernel(Geom g, Excha
         double m0 = mx[cidx], m1 = my[cidx], m2 = mz[cidx];
         double e = E[cidx], er = Er[cidx];
         double f0 = Fx[cidx], f1 = Fy[cidx], f2 = Fz[cidx];
-        const int rc = exchange_cell(kc, dt, rho[cidx], m0, m1, m2, e, er, f0, f1, f2, kP[cidx], kR[cidx], iters);
+        const double S = src ? dt * src[cidx] : 0.0;              // eq 27: energy added during the substep (X13)
+        const int rc = exchange_cell(kc, dt, rho[cidx], m0, m1, m2, e, er, f0, f1, f2, kP[cidx], kR[cidx], S, iters);
         fail = (rc == 4);
         bad = (rc == 5);
         if (!kc.static_matter) { mx[cidx] = m0; my[cidx] = m1; mz[cidx] = m2; }
@@ -74,7 +75,8 @@ __global__ void __launch_bounds__(128, QK_EX_MINB) exchange_kernel(Geom g, Excha
 
 int launch_exchange(const Geom &g, const PhysConsts &pc, double dt, const double *rho, double *mx, double *my,
                     double *mz, double *E, double *Er, double *Fx, double *Fy, double *Fz, const double *kP,
-                    const double *kR, Hydro5 Wout, Rad4p Sout, Counters *ctr, StateCache *cache, cudaStream_t st)
+                    const double *kR, const double *src, Hydro5 Wout, Rad4p Sout, Counters *ctr, StateCache *cache,
+                    cudaStream_t st)
 {
     ExchangeConsts kc;
     kc.c = pc.c; kc.c_hat = pc.c_hat; kc.a_rad = pc.a_rad; kc.kB_mu = pc.kB_mu; kc.gamma = pc.gamma;
@@ -83,7 +85,7 @@ int launch_exchange(const Geom &g, const PhysConsts &pc, double dt, const double
     kc.literal_stop = (pc.flags & QK_FLAG_NEWTON_LITERAL) != 0;
     kc.static_matter = (pc.flags & QK_FLAG_STATIC_MATTER) != 0;
     dim3 grid((g.nx + 127) / 128, g.ny, g.nz);
-    exchange_kernel<<<grid, 128, 0, st>>>(g, kc, dt, rho, mx, my, mz, E, Er, Fx, Fy, Fz, kP, kR, Wout, Sout, ctr, cache);
+    exchange_kernel<<<grid, 128, 0, st>>>(g, kc, dt, rho, mx, my, mz, E, Er, Fx, Fy, Fz, kP, kR, src, Wout, Sout, ctr, cache);
     return 1;
 }
 

@@ -47,6 +47,7 @@ struct qk_ctx {
     // cells), and whether it / the cached CFL speed still describe the state
     int w_cur, s_cur;
     bool w_valid, s_valid, smax_valid;
+    bool has_source;       // QK_SRC was set: the exchange reads it (otherwise S = 0 and the field is never touched)
     int path;              // QK_PATH_*
     // z-slab decomposition: inter-rank faces, the caller's halo mover, and the field list of the fill in progress
     unsigned ext_faces;
@@ -371,7 +372,8 @@ int do_exchange(qk_ctx *c, double dt)
     }
     Scope sc(c, K_EXCHANGE);
     sc.done(launch_exchange(c->g, c->pc, dt, s[QK_RHO], s[QK_MX], s[QK_MY], s[QK_MZ], s[QK_E], s[QK_ER], s[QK_FX],
-                            s[QK_FY], s[QK_FZ], s[QK_KAPPA_P], s[QK_KAPPA_R], W, S, c->ctr, c->cache, c->stream));
+                            s[QK_FY], s[QK_FZ], s[QK_KAPPA_P], s[QK_KAPPA_R], c->has_source ? s[QK_SRC] : nullptr, W, S, c->ctr,
+                            c->cache, c->stream));
     c->w_valid = sweep;
     c->s_valid = sweep;
     c->smax_valid = sweep;
@@ -413,7 +415,7 @@ int qk_init(int nx, int ny, int nz, double dx, double gamma, double c_hat, doubl
     x->pc.a_rad = 1.0; x->pc.kB_mu = 1.0; x->pc.eos_alpha = 0.0; x->pc.cfl = 0.3; x->pc.newton_tol = 1e-10;
     x->pc.newton_maxit = 400; x->pc.nsub_max = 10; x->pc.flags = QK_FLAG_TAU_CORR; x->pc.bc = boundary;
     x->stream = nullptr; x->device = dev; x->base = nullptr; x->bytes = 0; x->owns = false; x->ready = false;
-    x->path = QK_PATH_SWEEP; x->w_cur = 0; x->s_cur = 0; x->w_valid = false; x->s_valid = false; x->smax_valid = false;
+    x->path = QK_PATH_SWEEP; x->w_cur = 0; x->s_cur = 0; x->w_valid = false; x->s_valid = false; x->smax_valid = false; x->has_source = false;
     x->ext_faces = 0; x->halo_fn = nullptr; x->halo_user = nullptr; x->pending.n = 0; x->in_halo_cb = false;
     x->launches = 0; x->last_nsub = 0; x->profiling = false;
     *out = x;
@@ -489,7 +491,8 @@ int qk_set_state(qk_ctx *c, int field, const double *interior)
     if (!c || field < 0 || field >= QK_NFIELDS || !interior) return QK_EINVAL;
     int rc = ensure_storage(c);
     if (rc) return rc;
-    c->w_valid = false; c->s_valid = false; c->smax_valid = false;
+    if (field == QK_SRC) c->has_source = true;
+    else { c->w_valid = false; c->s_valid = false; c->smax_valid = false; }
     rc = copy_interior(c, c->state[field], const_cast<double *>(interior), true);
     // pageable host memory may be reused by the caller as soon as we return
     if (rc == QK_OK && !is_device_ptr(interior) && cudaStreamSynchronize(c->stream) != cudaSuccess) rc = QK_ECUDA;
@@ -511,7 +514,8 @@ int qk_set_raw(qk_ctx *c, int field, const double *with_ghosts)
     if (!c || field < 0 || field >= QK_NFIELDS || !with_ghosts) return QK_EINVAL;
     int rc = ensure_storage(c);
     if (rc) return rc;
-    c->w_valid = false; c->s_valid = false; c->smax_valid = false;
+    if (field == QK_SRC) c->has_source = true;
+    else { c->w_valid = false; c->s_valid = false; c->smax_valid = false; }
     if (cudaMemcpyAsync(c->state[field], with_ghosts, (size_t)c->g.ntot * sizeof(double), cudaMemcpyDefault,
                         c->stream) != cudaSuccess) return QK_ECUDA;
     return cudaStreamSynchronize(c->stream) == cudaSuccess ? QK_OK : QK_ECUDA;
@@ -534,7 +538,7 @@ int qk_fill_boundary(qk_ctx *c, int which)
     if (rc) return rc;
     double *list[QK_NFIELDS];
     signed char comps[QK_NFIELDS];
-    static const signed char comp_of[QK_NFIELDS] = {-1, 0, 1, 2, -1, -1, 0, 1, 2, -1, -1};
+    static const signed char comp_of[QK_NFIELDS] = {-1, 0, 1, 2, -1, -1, 0, 1, 2, -1, -1, -1};
     int n = 0;
     auto add = [&](int f) { list[n] = c->state[f]; comps[n] = comp_of[f]; ++n; };
     if (which & QK_FILL_HYDRO) for (int f = QK_RHO; f <= QK_E; ++f) add(f);

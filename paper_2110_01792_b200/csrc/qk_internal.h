@@ -112,7 +112,8 @@ int launch_rad_update(const Geom &g, double dtdx, int stage, CRad4p R, CRad4p R0
 
 int launch_exchange(const Geom &g, const PhysConsts &pc, double dt, const double *rho, double *mx, double *my,
                     double *mz, double *E, double *Er, double *Fx, double *Fy, double *Fz, const double *kP,
-                    const double *kR, Hydro5 Wout, Rad4p Sout, Counters *ctr, StateCache *cache, cudaStream_t st);
+                    const double *kR, const double *src, Hydro5 Wout, Rad4p Sout, Counters *ctr, StateCache *cache,
+                    cudaStream_t st);
 // Wout.rho == nullptr: exchange only; otherwise the kernel also writes the primitives W and the radiation
 // variables S = (E_r, f) of the updated cells and leaves the CFL speed of the new state in `cache`
 

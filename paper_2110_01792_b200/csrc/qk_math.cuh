@@ -285,14 +285,14 @@ struct ExchangeConsts {
 // 4 (Newton cap reached) or 5 (non-positive E_g or E_r afterwards); iters = Newton updates.
 QK_HD int exchange_cell(const ExchangeConsts &k, double dt, double rho, double &mx, double &my, double &mz,
                         double &E, double &Er, double &Fx, double &Fy, double &Fz, double kappaP, double kappaR,
-                        int &iters)
+                        double S, int &iters)
 {
     const double c_ratio = k.c / k.c_hat;
     const double m2_old = (mx * mx + my * my) + mz * mz;
     const double Ekin_old = 0.5 * m2_old / rho;
     const double Eg_old = E - Ekin_old;
     const double Er_old = Er;
-    const double Etot = Eg_old + c_ratio * Er_old;              // eq 38 with S = 0
+    const double Etot = Eg_old + c_ratio * (Er_old + S);        // eq 38
     const double coef = dt * rho * kappaP * k.c_hat;            // dt rho kappa_P c_hat (X1)
     const double Cv_ideal = rho * k.kB_mu / (k.gamma - 1.0);    // volumetric heat capacity (X2)
     double Eg = Eg_old, Erad = Er_old;
@@ -311,7 +311,7 @@ QK_HD int exchange_cell(const ExchangeConsts &k, double dt, double rho, double &
         const double T4 = T2 * T2;
         const double R = coef * (k.a_rad * T4 - Erad);                    // eq 28 (X1)
         const double FG = (Eg - Eg_old) + c_ratio * R;                    // eq 26
-        const double FR = (Erad - Er_old) - R;                            // eq 27, S = 0
+        const double FR = (Erad - Er_old) - (R + S);                      // eq 27
         const bool converged = (fabs(FG / Etot) < k.tol) && (fabs(c_ratio * FR / Etot) < k.tol);  // eq 36-37
         if (converged && k.literal_stop) { finished = true; break; }
         const double dR_dEg = coef * (4.0 * k.a_rad * (T2 * T)) / Cv;     // eq 33, d kappa/dT = 0

@@ -328,6 +328,30 @@ def test_exchange_parity_and_counters(flags):
     g.close()
 
 
+def test_exchange_with_source_field():
+    """eq 27 / 38 with a per-cell source rate (QK_SRC, reading X13): parity with the oracle, and without the
+    field the result is the sourceless one (S = 0 leaves every bit as before)."""
+    params, fields = I.ragged_rhd()
+    rng = np.random.default_rng(8)
+    src = rng.uniform(0.0, 5.0, fields["Er"].shape) * fields["Er"].mean()
+    g = P.make_oracle(params, fields)
+    g.set_state(O.FIELDS.index("src"), src)
+    names = I.FIELDS[:9]
+    with P.make_gpu(params, fields) as ctx, P.make_gpu(params, fields) as plain:
+        ctx.qk_set_state(B.FIELDS.index("src"), src)
+        dt = 0.5 * g.cfl_dt()
+        for _ in range(3):
+            assert g.exchange(dt) == 0
+            ctx.qk_exchange(dt)
+            plain.qk_exchange(dt)
+        ref, got = g.get_all(names), ctx.get_all(names)
+        for n in names:
+            assert np.array_equal(ref[n], got[n]), n
+        assert ctx.qk_last_info()["newton_total_iters"] == g.info()["newton_total_iters"]
+        assert not np.array_equal(plain.get_all(["Er"])["Er"], got["Er"])
+    g.close()
+
+
 def test_exchange_newton_cap_is_reported():
     params, fields = I.ragged_rhd()
     g = P.make_oracle(params, fields)
