@@ -155,6 +155,13 @@ double qk_cfl_dt(qk_ctx *ctx);
  * primitives, multidimensional flattening, PPM face states, HLLC fluxes, unsplit update. */
 int qk_hydro_step(qk_ctx *ctx, double dt);
 
+/* The same step with the timestep of eq 21 (qk_cfl_dt's formula and CFL number) evaluated ON THE DEVICE from the
+ * signal speed the previous step left there: nothing is read back, the launch queue never drains.  qk_last_dt
+ * returns the dt that was used (synchronises).  Sweep path only (QK_EINVAL otherwise).  If the state is bad
+ * (rho <= 0 or P <= 0 somewhere) dt is NaN, the state becomes NaN and qk_last_info().status is QK_ESTATE. */
+int qk_hydro_step_cfl(qk_ctx *ctx);
+int qk_last_dt(qk_ctx *ctx, double *dt);
+
 /* SSP-RK2 explicit transport of (E_r, F_r) over dt, no exchange. */
 int qk_rad_transport(qk_ctx *ctx, double dt);
 

@@ -29,7 +29,7 @@ EXPORTS = [
     "qk_cfl_dt", "qk_hydro_step", "qk_rad_transport", "qk_exchange", "qk_rad_step", "qk_rhd_step",
     "qk_nsub_for", "qk_last_info", "qk_launch_count", "qk_set_path", "qk_set_profiling",
     "qk_kernel_class_count", "qk_kernel_class_name", "qk_kernel_times", "qk_version", "qk_fp64_probe",
-    "qk_selftest_divsqrt", "qk_set_eos", "qk_set_halo_exchange", "qk_halo_doubles", "qk_halo_pack", "qk_halo_unpack",
+    "qk_selftest_divsqrt", "qk_set_eos", "qk_hydro_step_cfl", "qk_last_dt", "qk_set_halo_exchange", "qk_halo_doubles", "qk_halo_pack", "qk_halo_unpack",
 ]
 
 
@@ -77,6 +77,8 @@ def lib():
         "qk_fill_boundary": (i, [p, i]),
         "qk_cfl_dt": (d, [p]),
         "qk_hydro_step": (i, [p, d]),
+        "qk_hydro_step_cfl": (i, [p]),
+        "qk_last_dt": (i, [p, C.POINTER(d)]),
         "qk_rad_transport": (i, [p, d]),
         "qk_exchange": (i, [p, d]),
         "qk_rad_step": (i, [p, d]),
@@ -248,6 +250,14 @@ class Context:
 
     def qk_hydro_step(self, dt):
         _check(self.L.qk_hydro_step(self.h, dt), "qk_hydro_step")
+
+    def qk_hydro_step_cfl(self):
+        _check(self.L.qk_hydro_step_cfl(self.h), "qk_hydro_step_cfl")
+
+    def qk_last_dt(self):
+        out = C.c_double()
+        _check(self.L.qk_last_dt(self.h, C.byref(out)), "qk_last_dt")
+        return float(out.value)
 
     def qk_rad_transport(self, dt):
         _check(self.L.qk_rad_transport(self.h, dt), "qk_rad_transport")

@@ -49,6 +49,31 @@ __global__ void __launch_bounds__(256) cfl_max_speed_kernel(Geom g, double gamma
     }
 }
 
+// eq 21 (and the N_sub,max limit) on the device, same operations as qk_cfl_dt does on the host
+__global__ void dt_from_cache_kernel(const StateCache *cache, DeviceDt *out, double cfl, double dx, double c_hat, int nsub_max)
+{
+    double dt;
+    if (cache->cfl_bad != 0) {
+        dt = __longlong_as_double(0x7ff8000000000000LL);          // NaN: a cell has rho <= 0 or P <= 0
+    } else {
+        const double smax = __longlong_as_double((long long)cache->smax_bits);
+        dt = cfl * dx / smax;
+        if (c_hat > 0.0) {
+            const double dtr = (double)nsub_max * (cfl * dx / c_hat);
+            if (dtr < dt) dt = dtr;
+        }
+    }
+    out->dt = dt;
+    out->dtdx = dt / dx;
+}
+
+int launch_dt_from_cache(const StateCache *cache, DeviceDt *out, double cfl, double dx, double c_hat, int nsub_max,
+                         cudaStream_t st)
+{
+    dt_from_cache_kernel<<<1, 1, 0, st>>>(cache, out, cfl, dx, c_hat, nsub_max);
+    return 1;
+}
+
 int launch_cfl(const Geom &g, double gamma, CHydro5 U, StateCache *ctr, cudaStream_t st)
 {
     const long long ncell = (long long)g.nx * g.ny * g.nz;

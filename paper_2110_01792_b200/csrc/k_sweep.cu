@@ -304,9 +304,9 @@ static int sweep_len(int n_m, long long columns)
 template <class PH>
 static int launch_sweeps(const PH &ph, const Geom &g, double dtdx, int stage, FieldsRW<PH::NV> D, FieldsRO<PH::NV> U,
                          FieldsRO<PH::NV> U0, FieldsRW<PH::NV> out, FieldsRW<PH::NV> pout, Counters *ctr,
-                         StateCache *cache, cudaStream_t st, int which)
+                         StateCache *cache, cudaStream_t st, int which, const double *dtdx_dev = nullptr)
 {
-    const RkArgs rk{dtdx, stage};
+    const RkArgs rk{dtdx, stage, dtdx_dev};
     int n = 0;
     if (which & 1) {
         constexpr int rows = SW_XROWS * SW_XNROW;
@@ -332,7 +332,7 @@ static int launch_sweeps(const PH &ph, const Geom &g, double dtdx, int stage, Fi
 
 int launch_hydro_sweeps(const Geom &g, double gamma, unsigned scheme, double dtdx, int stage, CHydro5 W,
                         const double *chi, Hydro5 D, CHydro5 U, CHydro5 U0, Hydro5 out, Hydro5 Wout, Counters *ctr,
-                        StateCache *cache, cudaStream_t st, int which)
+                        StateCache *cache, cudaStream_t st, int which, const double *dtdx_dev)
 {
     FieldsRW<5> d{{D.rho, D.mx, D.my, D.mz, D.E}}, o{{out.rho, out.mx, out.my, out.mz, out.E}};
     FieldsRO<5> u{{U.rho, U.mx, U.my, U.mz, U.E}}, u0{{U0.rho, U0.mx, U0.my, U0.mz, U0.E}};
@@ -340,7 +340,7 @@ int launch_hydro_sweeps(const Geom &g, double gamma, unsigned scheme, double dtd
     auto go = [&](auto ph) {
         ph.w[0] = W.rho; ph.w[1] = W.mx; ph.w[2] = W.my; ph.w[3] = W.mz; ph.w[4] = W.E;
         ph.chi = chi; ph.gamma = gamma;
-        return launch_sweeps(ph, g, dtdx, stage, d, u, u0, o, wo, ctr, cache, st, which);
+        return launch_sweeps(ph, g, dtdx, stage, d, u, u0, o, wo, ctr, cache, st, which, dtdx_dev);
     };
     return (scheme & QK_FLAG_PLM) ? go(HydroPhT<1>()) : go(HydroPhT<0>());
 }

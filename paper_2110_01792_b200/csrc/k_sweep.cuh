@@ -52,7 +52,8 @@ constexpr int SW_XROWS = QK_SW_XROWS; // rows (warps) per CTA in the x sweep
 template <int NV> struct FieldsRW { double *f[NV]; };
 template <int NV> struct FieldsRO { const double *f[NV]; };
 
-struct RkArgs { double dtdx; int stage; };
+// dtdx_dev != nullptr: dt/dx is read from device memory (qk_hydro_step_cfl: the timestep never visits the host)
+struct RkArgs { double dtdx; int stage; const double *dtdx_dev; };
 
 __device__ __forceinline__ void sweep_count(Counters *ctr, int nfall, int nguard)
 {
@@ -152,6 +153,7 @@ __global__ void __launch_bounds__(SW_NT, MODE == 2 ? QK_SW_MINB2 : QK_SW_MINB1) 
                                                             StateCache *cache)
 {
     constexpr int NV = PH::NV;
+    const double dtdx = (MODE == 2 && rk.dtdx_dev) ? __ldg(rk.dtdx_dev) : rk.dtdx;
     typename PH::Tail tail;                             // per-thread reduction state of the MODE 2 epilogue
     __shared__ double ring[5 * SW_NR * SW_NT];          // [slot][var][thread], thread-private columns
     const int tid = threadIdx.x;
@@ -237,7 +239,7 @@ __global__ void __launch_bounds__(SW_NT, MODE == 2 ? QK_SW_MINB2 : QK_SW_MINB1) 
                 if (MODE == 1) {
                     D.f[v][cidx] = div;
                 } else {
-                    const double us = u[v] - rk.dtdx * div;
+                    const double us = u[v] - dtdx * div;
                     fresh[v] = rk.stage == 0 ? us : 0.5 * u0[v] + 0.5 * us;
                     out.f[v][cidx] = fresh[v];
                 }

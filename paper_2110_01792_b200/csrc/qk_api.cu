@@ -43,6 +43,7 @@ struct qk_ctx {
     double *scratch[N_SCRATCH_REF];
     Counters *ctr;
     StateCache *cache;
+    DeviceDt *ddt;         // device-resident timestep of qk_hydro_step_cfl
     // sweep path: which scratch set holds the reconstruction variables of the current state (interior
     // cells), and whether it / the cached CFL speed still describe the state
     int w_cur, s_cur;
@@ -82,6 +83,7 @@ int carve(qk_ctx *c)
     for (int f = 0; f < N_SCRATCH_REF; ++f) { c->scratch[f] = p; p += fs; }
     c->ctr = (Counters *)p;
     c->cache = (StateCache *)((char *)p + 128);
+    c->ddt = (DeviceDt *)((char *)p + 192);
     // zero everything once so ghost cells and unused corners are defined
     if (cudaMemsetAsync(c->base, 0, c->bytes, c->stream) != cudaSuccess) return QK_ECUDA;
     c->ready = true;
@@ -218,7 +220,7 @@ void hydro_stage_fused(qk_ctx *c, double dtdx, int stage, double *const *U, doub
 // here for every cell from the ghost-filled U).  The z sweep writes the updated state and its primitives
 // W_out (interior), and after the last stage the CFL speed of the new state.
 void hydro_stage_sweep(qk_ctx *c, double dtdx, int stage, double *const *U, double *const *U0, double *const *out,
-                       double *const *W, double *const *Wout, bool w_ready)
+                       double *const *W, double *const *Wout, bool w_ready, const double *dtdx_dev)
 {
     const Geom &g = c->g;
     double *const *D = &c->scratch[SC_D];
@@ -237,7 +239,7 @@ void hydro_stage_sweep(qk_ctx *c, double dtdx, int stage, double *const *U, doub
     for (int d = 0; d < 3; ++d) {
         Scope s(c, K_HYDRO_SWEEP_X + d);
         s.done(launch_hydro_sweeps(g, c->pc.gamma, c->pc.flags, dtdx, stage, ch5(W), c->chi, h5(D), ch5(U), ch5(U0), h5(out), h5(Wout),
-                                   c->ctr, c->cache, c->stream, 1 << d));
+                                   c->ctr, c->cache, c->stream, 1 << d, dtdx_dev));
     }
 }
 
@@ -254,7 +256,7 @@ bool scheme_supported(const qk_ctx *c)
     return c->path == QK_PATH_SWEEP || !(c->pc.flags & (QK_FLAG_PLM | QK_FLAG_EDDINGTON));
 }
 
-int do_hydro_step(qk_ctx *c, double dt)
+int do_hydro_step(qk_ctx *c, double dt, const double *dtdx_dev = nullptr)
 {
     if (!scheme_supported(c)) return QK_EINVAL;
     const double dtdx = dt / c->pc.dx;
@@ -263,9 +265,9 @@ int do_hydro_step(qk_ctx *c, double dt)
     if (c->path == QK_PATH_SWEEP) {
         double *const *W0 = &c->scratch[c->w_cur ? SC_WB : SC_WA];
         double *const *W1 = &c->scratch[c->w_cur ? SC_WA : SC_WB];
-        hydro_stage_sweep(c, dtdx, 0, Un, Un, U1, W0, W1, c->w_valid);
+        hydro_stage_sweep(c, dtdx, 0, Un, Un, U1, W0, W1, c->w_valid, dtdx_dev);
         cudaMemsetAsync(c->cache, 0, sizeof(StateCache), c->stream);
-        hydro_stage_sweep(c, dtdx, 1, U1, Un, Un, W1, W0, true);
+        hydro_stage_sweep(c, dtdx, 1, U1, Un, Un, W1, W0, true, dtdx_dev);
         c->w_valid = true;               // W0 = primitives of the new state, cache = its CFL speed
         c->smax_valid = true;
     } else {
@@ -602,6 +604,39 @@ int qk_hydro_step(qk_ctx *c, double dt)
     reset_counters(c);
     c->last_nsub = 0;
     return do_hydro_step(c, dt);
+}
+
+int qk_hydro_step_cfl(qk_ctx *c)
+{
+    if (!c) return QK_EINVAL;
+    int rc = ensure_storage(c);
+    if (rc) return rc;
+    if (c->path != QK_PATH_SWEEP) return QK_EINVAL;
+    reset_counters(c);
+    c->last_nsub = 0;
+    if (!c->smax_valid) {
+        cudaMemsetAsync(c->cache, 0, sizeof(StateCache), c->stream);
+        Scope s(c, K_CFL);
+        s.done(launch_cfl(c->g, c->pc.gamma, ch5(&c->state[QK_RHO]), c->cache, c->stream));
+        c->smax_valid = true;
+    }
+    {
+        Scope s(c, K_CFL);
+        s.done(launch_dt_from_cache(c->cache, c->ddt, c->pc.cfl, c->pc.dx, c->pc.c_hat, c->pc.nsub_max, c->stream));
+    }
+    return do_hydro_step(c, 1.0, &c->ddt->dtdx);
+}
+
+int qk_last_dt(qk_ctx *c, double *dt)
+{
+    if (!c || !dt) return QK_EINVAL;
+    int rc = ensure_storage(c);
+    if (rc) return rc;
+    DeviceDt h;
+    if (cudaMemcpyAsync(&h, c->ddt, sizeof(h), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+        cudaStreamSynchronize(c->stream) != cudaSuccess) { cudaGetLastError(); return QK_ECUDA; }
+    *dt = h.dt;
+    return QK_OK;
 }
 
 int qk_rad_transport(qk_ctx *c, double dt)

@@ -51,6 +51,12 @@ struct StateCache {
     long long cfl_bad;                 // interior cells with rho<=0 or P<=0
 };
 
+// Timestep kept on the device (qk_hydro_step_cfl): eq 21 evaluated from the cached signal speed by a one-thread
+// kernel, read by the z sweeps.  Lives beside StateCache, outside the part that is cleared between RK stages.
+struct DeviceDt { double dt, dtdx; };
+int launch_dt_from_cache(const StateCache *cache, DeviceDt *out, double cfl, double dx, double c_hat, int nsub_max,
+                         cudaStream_t st);
+
 // Kernel classes for per-kernel timing (qk_kernel_times) -- one id per __global__ function family.
 enum KClass { K_FILL = 0, K_CFL, K_PRIM, K_FLATTEN, K_HYDRO_FLUX, K_HYDRO_UPDATE, K_HYDRO_STAGE,
               K_RAD_PRIM, K_RAD_FLUX, K_RAD_UPDATE, K_RAD_STAGE, K_EXCHANGE,
@@ -97,7 +103,7 @@ int launch_rad_stage(const Geom &g, const PhysConsts &pc, double dtdx, int stage
 // sweep path (k_sweep.cu); `which` bit 0 = x sweep, bit 1 = y sweep, bit 2 = z sweep + RK update
 int launch_hydro_sweeps(const Geom &g, double gamma, unsigned scheme, double dtdx, int stage, CHydro5 W,
                         const double *chi, Hydro5 D, CHydro5 U, CHydro5 U0, Hydro5 out, Hydro5 Wout, Counters *ctr,
-                        StateCache *cache, cudaStream_t st, int which);
+                        StateCache *cache, cudaStream_t st, int which, const double *dtdx_dev);
 int launch_chi_two_pass(const Geom &g, double gamma, CHydro5 W, double *cx, double *cy, double *cz, double *chi,
                         cudaStream_t st);
 int launch_rad_sweeps(const Geom &g, const PhysConsts &pc, double dtdx, int stage, CRad4p S, const double *rho,

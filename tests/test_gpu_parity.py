@@ -183,6 +183,28 @@ def test_hydro_sedov_small_bitwise():
     print("sedov mismatching cells:", P.count_mismatch(*res[8], I.FIELDS[:5]))
 
 
+def test_device_resident_timestep_is_the_host_one():
+    """qk_hydro_step_cfl (eq 21 evaluated on the device) walks exactly the trajectory of qk_cfl_dt + qk_hydro_step."""
+    params, fields = I.ragged_hydro(seed=5)
+    with P.make_gpu(params, fields) as a, P.make_gpu(params, fields) as b:
+        for _ in range(6):
+            dt = a.qk_cfl_dt()
+            a.qk_hydro_step(dt)
+            b.qk_hydro_step_cfl()
+            assert b.qk_last_dt() == dt
+        ua, ub = a.get_all(I.FIELDS[:5]), b.get_all(I.FIELDS[:5])
+        for n in I.FIELDS[:5]:
+            assert np.array_equal(ua[n], ub[n]), n
+        assert a.qk_cfl_dt() == b.qk_cfl_dt()
+        # after an outside change of the state the cached speed is recomputed
+        b.qk_set_state(4, 2.0 * ub["E"])
+        a.qk_set_state(4, 2.0 * ub["E"])
+        dt = a.qk_cfl_dt()
+        a.qk_hydro_step(dt)
+        b.qk_hydro_step_cfl()
+        assert b.qk_last_dt() == dt and np.array_equal(a.qk_get_state(0), b.qk_get_state(0))
+
+
 def test_side_stream_and_two_contexts():
     """qk_set_stream: all work of a context goes to the stream it was given (a non-default torch stream here),
     and two contexts with different boxes advance independently (no global state in the library)."""
