@@ -20,7 +20,7 @@ _LIB = os.path.join(_HERE, "libqk_oracle.so")
 
 NG = 4
 FIELDS = ["rho", "mx", "my", "mz", "E", "Er", "Fx", "Fy", "Fz", "kappaP", "kappaR", "src"]
-BC_PERIODIC, BC_OUTFLOW, BC_REFLECTING = 0, 1, 2
+BC_PERIODIC, BC_OUTFLOW, BC_REFLECTING, BC_FIXED = 0, 1, 2, 3
 FLAG_TAU_CORR, FLAG_STATIC_MATTER, FLAG_NEWTON_LITERAL = 1, 2, 4
 FLAG_PLM, FLAG_EDDINGTON = 8, 16
 EOS_IDEAL, EOS_ALPHA_T3 = 0, 1
@@ -57,6 +57,7 @@ def lib():
         "orc_set_constants": (None, [p, d, d]),
         "orc_set_params": (None, [p, d, d, i, i, u]),
         "orc_set_eos": (None, [p, i, d]),
+        "orc_set_face_bc": (i, [p, np.ctypeslib.ndpointer(dtype=np.int32, flags="C_CONTIGUOUS")]),
         "orc_set_field": (None, [p, i, dp]),
         "orc_get_field": (None, [p, i, dp]),
         "orc_get_raw": (None, [p, i, dp]),
@@ -119,6 +120,11 @@ class Grid:
 
     def set_params(self, cfl=0.3, newton_tol=1e-10, newton_maxit=400, nsub_max=10, flags=FLAG_TAU_CORR):
         self.L.orc_set_params(self.h, cfl, newton_tol, newton_maxit, nsub_max, flags)
+
+    def set_face_bc(self, bc6):
+        """Per-face boundary types (x-lo, x-hi, y-lo, y-hi, z-lo, z-hi)."""
+        rc = self.L.orc_set_face_bc(self.h, np.ascontiguousarray(bc6, dtype=np.int32))
+        assert rc == 0, "periodic must be set on both faces of an axis"
 
     def set_eos(self, eos, alpha=0.0):
         self.L.orc_set_eos(self.h, eos, alpha)

@@ -26,6 +26,7 @@ orc_grid *orc_create(int nx, int ny, int nz, double dx, double gamma, double c_h
     if (!g) return NULL;
     g->nx = nx; g->ny = ny; g->nz = nz;
     g->dx = dx; g->gamma = gamma; g->c_hat = c_hat; g->c = c; g->bc = bc;
+    for (int f = 0; f < 6; ++f) g->face_bc[f] = bc;
     g->a_rad = 1.0; g->kB_mu = 1.0;
     g->cfl = 0.3; g->newton_tol = 1e-10; g->newton_maxit = 400; g->nsub_max = 10; /* PAPER.md:247,273 */
     g->flags = ORC_FLAG_TAU_CORR;
@@ -114,27 +115,39 @@ static int field_component(int field)
     }
 }
 
+int orc_set_face_bc(orc_grid *g, const int bc6[6])
+{
+    for (int a = 0; a < 3; ++a)
+        if ((bc6[2 * a] == ORC_BC_PERIODIC) != (bc6[2 * a + 1] == ORC_BC_PERIODIC)) return 1;
+    for (int f = 0; f < 6; ++f) g->face_bc[f] = bc6[f];
+    return 0;
+}
+
 static void fill_one(orc_grid *g, double *a, int comp)
 {
-    /* every ghost cell (faces, edges, corners) <- the interior cell its three axis
-     * indices map to; equivalent to filling x, then y, then z in sequence. */
-    for (int k = -ORC_NG; k < g->nz + ORC_NG; ++k) {
-        int ks = src_index(k, g->nz, g->bc);
-        for (int j = -ORC_NG; j < g->ny + ORC_NG; ++j) {
-            int js = src_index(j, g->ny, g->bc);
+    /* every ghost cell (faces, edges, corners) <- the interior cell its three axis indices map to, each axis by the
+     * rule of the face the index lies beyond; equivalent to filling x, then y, then z in sequence.  A ghost cell
+     * beyond a FIXED face is left as the caller stored it. */
+    const int n[3] = { g->nx, g->ny, g->nz };
+    for (int k = -ORC_NG; k < g->nz + ORC_NG; ++k)
+        for (int j = -ORC_NG; j < g->ny + ORC_NG; ++j)
             for (int i = -ORC_NG; i < g->nx + ORC_NG; ++i) {
-                int is = src_index(i, g->nx, g->bc);
-                if (is == i && js == j && ks == k) continue;
-                double v = a[idx(g, is, js, ks)];
-                if (g->bc == ORC_BC_REFLECTING) {
-                    int outside = (comp == 0 && (i < 0 || i >= g->nx)) || (comp == 1 && (j < 0 || j >= g->ny)) ||
-                                  (comp == 2 && (k < 0 || k >= g->nz));
-                    if (outside) v = -v;
+                const int idx3[3] = { i, j, k };
+                int src[3], fixed = 0, flip = 0, ghost = 0;
+                for (int ax = 0; ax < 3; ++ax) {
+                    int v = idx3[ax];
+                    src[ax] = v;
+                    if (v >= 0 && v < n[ax]) continue;
+                    ghost = 1;
+                    int bc = g->face_bc[2 * ax + (v < 0 ? 0 : 1)];
+                    if (bc == ORC_BC_FIXED) { fixed = 1; continue; }
+                    src[ax] = src_index(v, n[ax], bc);
+                    if (bc == ORC_BC_REFLECTING && comp == ax) flip = !flip;
                 }
-                a[idx(g, i, j, k)] = v;
+                if (!ghost || fixed) continue;
+                double val = a[idx(g, src[0], src[1], src[2])];
+                a[idx(g, i, j, k)] = flip ? -val : val;
             }
-        }
-    }
 }
 
 void orc_fill_field(orc_grid *g, int field) { fill_one(g, g->f[field], field_component(field)); }

@@ -40,7 +40,9 @@ enum { ORC_RHO = 0, ORC_MX, ORC_MY, ORC_MZ, ORC_E, ORC_ER, ORC_FX, ORC_FY, ORC_F
        ORC_KP, ORC_KR,
        ORC_SRC };   /* radiation energy source rate per cell: S of eq 27 is dt * src (reading X13) */
 enum { ORC_BC_PERIODIC = 0, ORC_BC_OUTFLOW = 1,
-       ORC_BC_REFLECTING = 2 };  /* solid wall: mirror image, normal momentum / flux component negated */
+       ORC_BC_REFLECTING = 2,
+       ORC_BC_FIXED = 3 };       /* Dirichlet: the ghost cells keep the values the caller stored (orc_set_raw);
+                                    PAPER.md:492, 518, 528; inflow boundaries 422, 464, 476 (B2) */  /* solid wall: mirror image, normal momentum / flux component negated */
 enum { ORC_FLAG_TAU_CORR = 1, ORC_FLAG_STATIC_MATTER = 2, ORC_FLAG_NEWTON_LITERAL = 4,
        ORC_FLAG_PLM = 8,          /* piecewise-linear reconstruction with the MC limiter */
        ORC_FLAG_EDDINGTON = 16 }; /* Eddington approximation chi = 1/3 (P_r = E_r/3)  */
@@ -50,7 +52,8 @@ enum { ORC_FILL_HYDRO = 1, ORC_FILL_RAD = 2, ORC_FILL_ALL = 7 }; /* bit 4: opaci
 typedef struct orc_grid {
     int nx, ny, nz;                 /* interior cells                                  */
     double dx, gamma, c_hat, c;
-    int bc;
+    int bc;                         /* boundary given to orc_create: all six faces       */
+    int face_bc[6];                 /* per face: x-lo, x-hi, y-lo, y-hi, z-lo, z-hi      */
     double a_rad, kB_mu;            /* radiation constant, k_B/(mu m_H)                */
     double cfl, newton_tol;
     int newton_maxit, nsub_max;
@@ -75,6 +78,7 @@ long long orc_ncells_total(const orc_grid *g);
 void   orc_set_constants(orc_grid *g, double a_rad, double kB_mu);
 void   orc_set_params(orc_grid *g, double cfl, double newton_tol, int newton_maxit, int nsub_max, unsigned flags);
 void   orc_set_eos(orc_grid *g, int eos, double alpha);
+int    orc_set_face_bc(orc_grid *g, const int bc6[6]);   /* 0 ok, 1 if periodic is not on both faces of an axis */
 void   orc_set_field(orc_grid *g, int field, const double *interior);
 void   orc_get_field(const orc_grid *g, int field, double *interior);
 void   orc_get_raw(const orc_grid *g, int field, double *with_ghosts);
