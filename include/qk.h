@@ -35,8 +35,10 @@ enum { QK_OK = 0, QK_EINVAL = 1, QK_ENOMEM = 2, QK_ECUDA = 3,
 
 enum { QK_BC_PERIODIC = 0,   /* PAPER.md:293, 572 */
        QK_BC_OUTFLOW = 1,    /* PAPER.md:464; zero-gradient copy of the nearest interior cell (H15) */
-       QK_BC_REFLECTING = 2 };/* PAPER.md:408, 438, 464; solid wall: mirror image, the wall-normal component of
-                                 rho v and F_r negated (B1) */
+       QK_BC_REFLECTING = 2, /* PAPER.md:408, 438, 464; solid wall: mirror image, the wall-normal component of
+                                rho v and F_r negated (B1) */
+       QK_BC_FIXED = 3 };    /* Dirichlet / inflow (PAPER.md:422, 464, 476, 492, 518, 528): the ghost cells beyond the
+                                face keep the values the caller stored with qk_set_raw (B2); sweep path only */
 
 /* field ids: conserved hydro U=(rho, rho v, E) (PAPER.md:114, 289), radiation moments
  * (E_r, F_r) (eq 11-12, PAPER.md:87-89), Planck- and Rosseland-type opacities per cell
@@ -104,6 +106,12 @@ int qk_set_stream(qk_ctx *ctx, void *cuda_stream);
 /* radiation constant a_r and k_B/(mu m_H) of the ideal-gas temperature
  * T = (gamma-1) E_g / (rho k_B/(mu m_H)) (X2). */
 int qk_set_constants(qk_ctx *ctx, double a_rad, double kB_over_mu_mH);
+
+/* Boundary type per face, in the order x-lo, x-hi, y-lo, y-hi, z-lo, z-hi (qk_init sets all six alike).  Periodic
+ * must be given on both faces of an axis (QK_EINVAL otherwise).  A ghost cell takes, axis by axis, the rule of the
+ * face its index lies beyond; a cell beyond any QK_BC_FIXED face is never written by the fill: store its values
+ * (all state fields, the whole ghost slab including edges and corners) with qk_set_raw before stepping. */
+int qk_set_face_boundaries(qk_ctx *ctx, const int *bc6);
 
 /* Equation of state of the gas in the EXCHANGE step: QK_EOS_IDEAL (default; T = (gamma-1) E_g / (rho k_B/(mu m_H)))
  * or QK_EOS_ALPHA_T3, E_g = alpha T^4 / 4 with volumetric heat capacity C_v = alpha T^3 (eq 55, PAPER.md:424-427;

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libqk.so")
 NG = 4
 FIELDS = ["rho", "mx", "my", "mz", "E", "Er", "Fx", "Fy", "Fz", "kappaP", "kappaR", "src"]
 QK_OK, QK_EINVAL, QK_ENOMEM, QK_ECUDA, QK_ENEWTON, QK_ESTATE = range(6)
-QK_BC_PERIODIC, QK_BC_OUTFLOW, QK_BC_REFLECTING = 0, 1, 2
+QK_BC_PERIODIC, QK_BC_OUTFLOW, QK_BC_REFLECTING, QK_BC_FIXED = 0, 1, 2, 3
 QK_FLAG_TAU_CORR, QK_FLAG_STATIC_MATTER, QK_FLAG_NEWTON_LITERAL = 1, 2, 4
 QK_FLAG_PLM, QK_FLAG_EDDINGTON = 8, 16
 QK_FILL_HYDRO, QK_FILL_RAD, QK_FILL_OPACITY, QK_FILL_ALL = 1, 2, 4, 7
@@ -29,7 +29,7 @@ EXPORTS = [
     "qk_cfl_dt", "qk_hydro_step", "qk_rad_transport", "qk_exchange", "qk_rad_step", "qk_rhd_step",
     "qk_nsub_for", "qk_last_info", "qk_launch_count", "qk_set_path", "qk_set_profiling",
     "qk_kernel_class_count", "qk_kernel_class_name", "qk_kernel_times", "qk_version", "qk_fp64_probe",
-    "qk_selftest_divsqrt", "qk_set_eos", "qk_hydro_step_cfl", "qk_last_dt", "qk_set_halo_exchange", "qk_halo_doubles", "qk_halo_pack", "qk_halo_unpack",
+    "qk_selftest_divsqrt", "qk_set_eos", "qk_set_face_boundaries", "qk_hydro_step_cfl", "qk_last_dt", "qk_set_halo_exchange", "qk_halo_doubles", "qk_halo_pack", "qk_halo_unpack",
 ]
 
 
@@ -70,6 +70,7 @@ def lib():
         "qk_set_constants": (i, [p, d, d]),
         "qk_set_params": (i, [p, d, d, i, i, u]),
         "qk_set_eos": (i, [p, i, d]),
+        "qk_set_face_boundaries": (i, [p, C.POINTER(C.c_int)]),
         "qk_set_state": (i, [p, i, p]),
         "qk_get_state": (i, [p, i, p]),
         "qk_set_raw": (i, [p, i, p]),
@@ -191,6 +192,10 @@ class Context:
 
     def qk_set_params(self, cfl=0.3, newton_tol=1e-10, newton_maxit=400, nsub_max=10, flags=QK_FLAG_TAU_CORR):
         _check(self.L.qk_set_params(self.h, cfl, newton_tol, newton_maxit, nsub_max, flags), "qk_set_params")
+
+    def qk_set_face_boundaries(self, bc6):
+        arr = (C.c_int * 6)(*[int(b) for b in bc6])
+        _check(self.L.qk_set_face_boundaries(self.h, arr), "qk_set_face_boundaries")
 
     def qk_set_eos(self, eos, alpha=0.0):
         _check(self.L.qk_set_eos(self.h, eos, alpha), "qk_set_eos")

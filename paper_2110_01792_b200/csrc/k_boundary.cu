@@ -30,7 +30,7 @@ __device__ __forceinline__ int wrap_index(int i, int n, int bc)
 
 // `ext` = QK_FACE_* bits of the z faces that border another rank's slab: their ghost planes already hold the
 // neighbour's cells at the interior (i, j) positions (qk_halo_unpack), so only their x / y images are filled.
-__global__ void __launch_bounds__(256) fill_ghost_kernel(Geom g, int bc, unsigned ext, FillList fl)
+__global__ void __launch_bounds__(256) fill_ghost_kernel(Geom g, FaceBc fb, unsigned ext, FillList fl)
 {
     const long long nZ = 2LL * NG * g.py * g.px;
     const long long nY = 2LL * NG * g.nz * g.px;
@@ -60,18 +60,32 @@ __global__ void __launch_bounds__(256) fill_ghost_kernel(Geom g, int bc, unsigne
             j = row - k * g.ny;
             i = ii < NG ? ii - NG : g.nx + (ii - NG);
         }
-        const bool k_ext = (k < 0 && (ext & QK_FACE_ZLO)) || (k >= g.nz && (ext & QK_FACE_ZHI));
+        // per axis: the rule of the face the index lies beyond (FaceBc: x-lo, x-hi, y-lo, y-hi, z-lo, z-hi)
+        const int idx3[3] = {i, j, k}, n3[3] = {g.nx, g.ny, g.nz};
+        int src3[3];
+        bool keep = false, out_refl[3] = {false, false, false};
+#pragma unroll
+        for (int ax = 0; ax < 3; ++ax) {
+            const int v = idx3[ax];
+            src3[ax] = v;
+            if (v >= 0 && v < n3[ax]) continue;
+            const int lohi = v < 0 ? 0 : 1;
+            if (ax == 2 && (ext & (lohi ? QK_FACE_ZHI : QK_FACE_ZLO))) continue;      // neighbour's planes: keep k
+            const int t_bc = fb.t[2 * ax + lohi];
+            if (t_bc == QK_BC_FIXED) { keep = true; continue; }                         // Dirichlet: caller's values
+            src3[ax] = wrap_index(v, n3[ax], t_bc);
+            out_refl[ax] = t_bc == QK_BC_REFLECTING;
+        }
         const int dst = g.at(i, j, k);
-        const int src = g.at(wrap_index(i, g.nx, bc), wrap_index(j, g.ny, bc), k_ext ? k : wrap_index(k, g.nz, bc));
-        if (src == dst) continue;
-        if (bc == QK_BC_REFLECTING) {
+        const int src = g.at(src3[0], src3[1], src3[2]);
+        if (keep || src == dst) continue;
+        if (out_refl[0] || out_refl[1] || out_refl[2]) {
             // the normal component of rho v / v / F_r / f changes sign across each wall the image lies beyond
-            const bool out[3] = {i < 0 || i >= g.nx, j < 0 || j >= g.ny, !k_ext && (k < 0 || k >= g.nz)};
 #pragma unroll 1
             for (int f = 0; f < fl.n; ++f) {
                 const double v = fl.f[f][src];
                 const int cm = fl.comp[f];
-                fl.f[f][dst] = (cm >= 0 && out[cm]) ? -v : v;
+                fl.f[f][dst] = (cm >= 0 && out_refl[cm]) ? -v : v;
             }
             continue;
         }
@@ -113,14 +127,14 @@ int launch_halo_copy(const Geom &g, int face_hi, int unpack, const FillList &fl,
     return 1;
 }
 
-int launch_fill(const Geom &g, int bc, unsigned ext, const FillList &fl, cudaStream_t st)
+int launch_fill(const Geom &g, const FaceBc &fb, unsigned ext, const FillList &fl, cudaStream_t st)
 {
     if (fl.n <= 0) return 0;
     const long long total = 2LL * NG * ((long long)g.py * g.px + (long long)g.nz * g.px + (long long)g.nz * g.ny);
     long long blocks = (total + 255) / 256;
     const long long cap = 148LL * 32;
     if (blocks > cap) blocks = cap;
-    fill_ghost_kernel<<<(unsigned)blocks, 256, 0, st>>>(g, bc, ext, fl);
+    fill_ghost_kernel<<<(unsigned)blocks, 256, 0, st>>>(g, fb, ext, fl);
     return 1;
 }
 

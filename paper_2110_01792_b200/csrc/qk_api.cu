@@ -48,6 +48,8 @@ struct qk_ctx {
     // cells), and whether it / the cached CFL speed still describe the state
     int w_cur, s_cur;
     bool w_valid, s_valid, smax_valid;
+    FaceBc fb;             // boundary type of each face (qk_init sets all six alike)
+    bool has_fixed;        // some face is QK_BC_FIXED: the ghost cells beyond it hold caller-supplied values
     bool has_source;       // QK_SRC was set: the exchange reads it (otherwise S = 0 and the field is never touched)
     int path;              // QK_PATH_*
     // z-slab decomposition: inter-rank faces, the caller's halo mover, and the field list of the fill in progress
@@ -180,7 +182,7 @@ void fill_fields(qk_ctx *c, double *const *fields, int n, const signed char *com
         c->halo_fn(c->halo_user, n);
         c->in_halo_cb = false;
     }
-    s.done(launch_fill(c->g, c->pc.bc, c->ext_faces, fl, c->stream));
+    s.done(launch_fill(c->g, c->fb, c->ext_faces, fl, c->stream));
 }
 
 // ---- hydro: SSP-RK2 ------------------------------------------------------------------
@@ -229,7 +231,10 @@ void hydro_stage_sweep(qk_ctx *c, double dtdx, int stage, double *const *U, doub
     } else {
         fill_fields(c, U, 5);
         Scope s(c, K_PRIM);
-        s.done(launch_prim(g, c->pc.gamma, ch5(U), h5(W), c->ctr, c->stream));
+        int n = launch_prim(g, c->pc.gamma, ch5(U), h5(W), c->ctr, c->stream);
+        // ghost cells beyond a Dirichlet face are never refilled: the other W set needs their primitives too
+        if (c->has_fixed) n += launch_prim(g, c->pc.gamma, ch5(U), h5(Wout), c->ctr, c->stream);
+        s.done(n);
     }
     {
         Scope s(c, K_FLATTEN);
@@ -250,10 +255,10 @@ void hydro_stage(qk_ctx *c, double dtdx, int stage, double *const *U, double *co
     else hydro_stage_unfused(c, dtdx, stage, U, U0, out);
 }
 
-// the PLM / Eddington variants exist in the sweep path only
+// the PLM / Eddington variants and Dirichlet faces exist in the sweep path only
 bool scheme_supported(const qk_ctx *c)
 {
-    return c->path == QK_PATH_SWEEP || !(c->pc.flags & (QK_FLAG_PLM | QK_FLAG_EDDINGTON));
+    return c->path == QK_PATH_SWEEP || (!(c->pc.flags & (QK_FLAG_PLM | QK_FLAG_EDDINGTON)) && !c->has_fixed);
 }
 
 int do_hydro_step(qk_ctx *c, double dt, const double *dtdx_dev = nullptr)
@@ -322,7 +327,9 @@ void rad_stage_sweep(qk_ctx *c, double dtdx, int stage, double *const *R, double
     fill_fields(c, list, n);
     if (!s_ready) {
         Scope s(c, K_RAD_PRIM);
-        s.done(launch_rad_prim(g, c->pc.c, cr4(R), r4(S), c->ctr, c->stream));
+        int n = launch_rad_prim(g, c->pc.c, cr4(R), r4(S), c->ctr, c->stream);
+        if (c->has_fixed) n += launch_rad_prim(g, c->pc.c, cr4(R), r4(Sout), c->ctr, c->stream);
+        s.done(n);
     }
     for (int d = 0; d < 3; ++d) {
         Scope s(c, K_RAD_SWEEP_X + d);
@@ -405,7 +412,7 @@ int qk_init(int nx, int ny, int nz, double dx, double gamma, double c_hat, doubl
     if (!out) return QK_EINVAL;
     *out = nullptr;
     if (nx < 1 || ny < 1 || nz < 1 || !(dx > 0.0) || !(gamma > 1.0) || c_hat < 0.0 || c < 0.0) return QK_EINVAL;
-    if (boundary != QK_BC_PERIODIC && boundary != QK_BC_OUTFLOW && boundary != QK_BC_REFLECTING) return QK_EINVAL;
+    if (boundary < QK_BC_PERIODIC || boundary > QK_BC_FIXED) return QK_EINVAL;
     if ((long long)(nx + 2 * NG) * (ny + 2 * NG) * (nz + 2 * NG) > 2000000000LL) return QK_EINVAL;
     if (ny + 4 > 65535 || nz + 4 > 65535) return QK_EINVAL;
     int dev = 0;
@@ -417,7 +424,8 @@ int qk_init(int nx, int ny, int nz, double dx, double gamma, double c_hat, doubl
     x->pc.a_rad = 1.0; x->pc.kB_mu = 1.0; x->pc.eos_alpha = 0.0; x->pc.cfl = 0.3; x->pc.newton_tol = 1e-10;
     x->pc.newton_maxit = 400; x->pc.nsub_max = 10; x->pc.flags = QK_FLAG_TAU_CORR; x->pc.bc = boundary;
     x->stream = nullptr; x->device = dev; x->base = nullptr; x->bytes = 0; x->owns = false; x->ready = false;
-    x->path = QK_PATH_SWEEP; x->w_cur = 0; x->s_cur = 0; x->w_valid = false; x->s_valid = false; x->smax_valid = false; x->has_source = false;
+    x->path = QK_PATH_SWEEP; x->w_cur = 0; x->s_cur = 0; x->w_valid = false; x->s_valid = false; x->smax_valid = false; x->has_source = false; x->has_fixed = boundary == QK_BC_FIXED;
+    for (int f = 0; f < 6; ++f) x->fb.t[f] = boundary;
     x->ext_faces = 0; x->halo_fn = nullptr; x->halo_user = nullptr; x->pending.n = 0; x->in_halo_cb = false;
     x->launches = 0; x->last_nsub = 0; x->profiling = false;
     *out = x;
@@ -462,6 +470,19 @@ int qk_set_constants(qk_ctx *c, double a_rad, double kB_over_mu_mH)
 {
     if (!c || !(a_rad >= 0.0) || !(kB_over_mu_mH > 0.0)) return QK_EINVAL;
     c->pc.a_rad = a_rad; c->pc.kB_mu = kB_over_mu_mH;
+    return QK_OK;
+}
+
+int qk_set_face_boundaries(qk_ctx *c, const int *bc6)
+{
+    if (!c || !bc6) return QK_EINVAL;
+    for (int f = 0; f < 6; ++f)
+        if (bc6[f] < QK_BC_PERIODIC || bc6[f] > QK_BC_FIXED) return QK_EINVAL;
+    for (int a = 0; a < 3; ++a)
+        if ((bc6[2 * a] == QK_BC_PERIODIC) != (bc6[2 * a + 1] == QK_BC_PERIODIC)) return QK_EINVAL;
+    c->has_fixed = false;
+    for (int f = 0; f < 6; ++f) { c->fb.t[f] = bc6[f]; c->has_fixed = c->has_fixed || bc6[f] == QK_BC_FIXED; }
+    c->w_valid = false; c->s_valid = false;
     return QK_OK;
 }
 

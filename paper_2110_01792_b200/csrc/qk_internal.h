@@ -82,7 +82,8 @@ struct CRad4p { const double *E, *Fx, *Fy, *Fz; };
 struct FillList { double *f[QK_NFIELDS]; signed char comp[QK_NFIELDS]; int n; };
 
 // ---- launchers (each enqueues on `st`; returns the number of kernels launched) -----------------
-int launch_fill(const Geom &g, int bc, unsigned ext_faces, const FillList &fl, cudaStream_t st);
+struct FaceBc { int t[6]; };      // QK_BC_* of the faces x-lo, x-hi, y-lo, y-hi, z-lo, z-hi
+int launch_fill(const Geom &g, const FaceBc &fb, unsigned ext_faces, const FillList &fl, cudaStream_t st);
 int launch_halo_copy(const Geom &g, int face_hi, int unpack, const FillList &fl, double *buf, cudaStream_t st);
 int launch_cfl(const Geom &g, double gamma, CHydro5 U, StateCache *cache, cudaStream_t st);
 

@@ -732,3 +732,113 @@ def test_gpu_leblanc_shock_tube():
     e_num = P[plateau] / ((g - 1) * rho[plateau])
     e_ex = p_ex[plateau] / ((g - 1) * rho_ex[plateau])
     assert np.abs(e_num / e_ex - 1.0).max() < 0.1
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-3: per-face boundaries and the Dirichlet (fixed ghost values) type
+# ------------------------------------------------------------------------------------------------
+def _pair_with_faces(params, faces):
+    g = O.Grid(params["nx"], params["ny"], params["nz"], params["dx"], params["gamma"],
+               c_hat=params.get("c_hat", 0.0), c=params.get("c", 0.0))
+    g.set_constants(params.get("a_rad", 1.0), params.get("kB_mu", 1.0))
+    g.set_params(cfl=params["cfl"], flags=params["flags"])
+    g.set_face_bc(faces)
+    ctx = B.Context(params["nx"], params["ny"], params["nz"], params["dx"], params["gamma"],
+                    params.get("c_hat", 0.0), params.get("c", 0.0))
+    ctx.qk_set_constants(params.get("a_rad", 1.0), params.get("kB_mu", 1.0))
+    ctx.qk_set_params(cfl=params["cfl"], flags=params["flags"])
+    ctx.qk_set_face_boundaries(faces)
+    return g, ctx
+
+
+def _ghosted(fields, rng, jitter=0.05):
+    """Interior from `fields`, ghost cells = a smooth-ish positive extension (edge values times 1 +- jitter)."""
+    out = {}
+    for n, a in fields.items():
+        p = np.pad(a, 4, mode="edge")
+        noise = 1.0 + jitter * rng.uniform(-1, 1, p.shape)
+        noise[4:-4, 4:-4, 4:-4] = 1.0
+        out[n] = np.ascontiguousarray(p * noise)
+    return out
+
+
+MIXED = [B.QK_BC_FIXED, B.QK_BC_OUTFLOW, B.QK_BC_PERIODIC, B.QK_BC_PERIODIC, B.QK_BC_REFLECTING, B.QK_BC_FIXED]
+
+
+def test_mixed_face_boundary_fill_bit_exact():
+    params, fields = I.ragged_rhd()
+    g, ctx = _pair_with_faces(params, MIXED)
+    raw = _ghosted(fields, np.random.default_rng(3))
+    with ctx:
+        for f, n in enumerate(I.FIELDS):
+            g.set_raw(f, raw[n])
+            ctx.qk_set_raw(f, raw[n])
+        g.fill_boundary(O.FILL_ALL)
+        ctx.qk_fill_boundary(B.QK_FILL_ALL)
+        for f in range(len(I.FIELDS)):
+            assert np.array_equal(np.asarray(g.get_raw(f)).reshape(-1).view(np.uint64),
+                                  np.asarray(ctx.qk_get_raw(f)).reshape(-1).view(np.uint64)), I.FIELDS[f]
+        with pytest.raises(B.QkError):
+            ctx.qk_set_face_boundaries([0, 1, 0, 0, 0, 0])
+    g.close()
+
+
+@pytest.mark.parametrize("kind", ["hydro", "rhd"])
+def test_steps_with_fixed_and_mixed_faces(kind):
+    params, fields = I.ragged_hydro() if kind == "hydro" else I.ragged_rhd()
+    g, ctx = _pair_with_faces(params, MIXED)
+    raw = _ghosted(fields, np.random.default_rng(5))
+    names = I.FIELDS[:5] if kind == "hydro" else I.FIELDS[:9]
+    with ctx:
+        for f, n in enumerate(I.FIELDS):
+            g.set_raw(f, raw[n])
+            ctx.qk_set_raw(f, raw[n])
+        for s in range(3):
+            dt = g.cfl_dt()
+            assert ctx.qk_cfl_dt() == dt
+            if kind == "hydro":
+                assert g.hydro_step(dt) == 0
+                ctx.qk_hydro_step(dt)
+            else:
+                assert g.rhd_step(dt) == 0
+                ctx.qk_rhd_step(dt)
+        ref, got = g.get_all(names), ctx.get_all(names)
+        for n in names:
+            assert np.array_equal(ref[n], got[n]), n
+        ctx.qk_set_path(B.QK_PATH_FUSED)                 # Dirichlet faces exist in the sweep path only
+        with pytest.raises(B.QkError):
+            ctx.qk_hydro_step(1e-5)
+    g.close()
+
+
+def test_gpu_beam_through_fixed_face_and_invariant_stream():
+    """The two physical pins of tests/test_oracle_boundaries.py straight on the CUDA path."""
+    g53 = 5.0 / 3.0
+    faces = [B.QK_BC_FIXED, B.QK_BC_FIXED, B.QK_BC_PERIODIC, B.QK_BC_PERIODIC, B.QK_BC_OUTFLOW, B.QK_BC_OUTFLOW]
+    with B.Context(12, 5, 4, 0.1, g53) as ctx:
+        ctx.qk_set_face_boundaries(faces)
+        rho, vx, P = 1.3, 4.0, 0.7
+        U = [rho, rho * vx, 0.0, 0.0, P / (g53 - 1) + 0.5 * rho * vx * vx]
+        for f, v in enumerate(U):
+            ctx.qk_set_raw(f, np.full((12, 13, 20), v))
+        for _ in range(10):
+            ctx.qk_hydro_step(ctx.qk_cfl_dt())
+        for f, v in enumerate(U):
+            assert np.all(ctx.qk_get_state(f) == v)
+    N, c, c_hat = 128, 1.0, 0.25
+    with B.Context(N, 1, 1, 1.0 / N, g53, c_hat, c) as ctx:
+        ctx.qk_set_params(flags=0)
+        ctx.qk_set_face_boundaries([B.QK_BC_FIXED, B.QK_BC_OUTFLOW, 0, 0, 0, 0])
+        i = np.arange(-4, N + 4)
+        Er = np.where(i < 0, 1.0, 1e-8)
+        shape_g = (9, 9, N + 8)
+        for name, a in (("Er", Er), ("Fx", c * Er), ("rho", np.ones_like(Er))):
+            ctx.qk_set_raw(B.FIELDS.index(name), np.broadcast_to(a, shape_g).copy())
+        dt, nsteps = 0.3 / N / c_hat, 200
+        for _ in range(nsteps):
+            ctx.qk_rad_transport(dt)
+        E = ctx.qk_get_state(5).ravel()
+        x = (np.arange(N) + 0.5) / N
+        front = c_hat * nsteps * dt
+        assert np.abs(E[x < front - 0.1] - 1.0).max() < 2e-2 and E[x > front + 0.1].max() < 1e-3
+        assert abs(x[np.nonzero(E > 0.5)[0][-1]] - front) < 0.03
