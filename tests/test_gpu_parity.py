@@ -842,3 +842,42 @@ def test_gpu_beam_through_fixed_face_and_invariant_stream():
         front = c_hat * nsteps * dt
         assert np.abs(E[x < front - 0.1] - 1.0).max() < 2e-2 and E[x > front + 0.1].max() < 1e-3
         assert abs(x[np.nonzero(E > 0.5)[0][-1]] - front) < 0.03
+
+
+# ------------------------------------------------------------------------------------------------
+# Full-size properties that hold at any size: conservation on the periodic 256^3 bench workloads
+# ------------------------------------------------------------------------------------------------
+def _sum(a):
+    return float(np.sum(a, dtype=np.longdouble))
+
+
+def test_full_size_conservation_config2_and_config4():
+    """on periodic grids the flux-form update conserves mass, momentum and energy, and the
+    exchange conserves rho v + F_r/(c c_hat) and E + (c/c_hat) E_r, to round-off -- at the bench's 256^3."""
+    params, fields = I.config2()
+    with P.make_gpu(params, fields) as ctx:
+        tot0 = [_sum(fields[n]) for n in I.FIELDS[:5]]
+        for _ in range(5):
+            ctx.qk_hydro_step(ctx.qk_cfl_dt())
+        got = ctx.get_all(I.FIELDS[:5])
+        assert ctx.qk_last_info()["status"] == 0
+    scale = [tot0[0], _sum(np.abs(fields["mx"])), _sum(np.abs(fields["my"])), _sum(np.abs(fields["mz"])), tot0[4]]
+    for n, t0, sc in zip(I.FIELDS[:5], tot0, scale):
+        assert abs(_sum(got[n]) - t0) < 1e-12 * sc, n
+    del got
+    params, fields = I.config4()
+    c, ch = params["c"], params["c_hat"]
+    with P.make_gpu(params, fields) as ctx:
+        for _ in range(3):
+            ctx.qk_rhd_step(ctx.qk_cfl_dt())
+        got = ctx.get_all(I.FIELDS[:9])
+        info = ctx.qk_last_info()
+    assert info["status"] == 0 and info["nsub"] == 1
+    assert abs(_sum(got["rho"]) - _sum(fields["rho"])) < 1e-12 * _sum(fields["rho"])
+    for m, f in (("mx", "Fx"), ("my", "Fy"), ("mz", "Fz")):
+        before = _sum(fields[m]) + _sum(fields[f]) / (c * ch)
+        after = _sum(got[m]) + _sum(got[f]) / (c * ch)
+        assert abs(after - before) < 1e-12 * _sum(np.abs(fields[m])), m
+    e0 = _sum(fields["E"]) + (c / ch) * _sum(fields["Er"])
+    e1 = _sum(got["E"]) + (c / ch) * _sum(got["Er"])
+    assert abs(e1 - e0) < 1e-12 * e0
