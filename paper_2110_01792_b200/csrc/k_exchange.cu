@@ -11,7 +11,7 @@
 namespace qk {
 
 #ifndef QK_EX_MINB
-#define QK_EX_MINB 6     // <= 85 registers: 1.09 -> 1.04 ms at 256^3; 8 spills into the Newton loop (1.45 ms)
+#define QK_EX_MINB 7     // <= 73 registers: 1.09 -> 1.02 ms at 256^3 (6: 1.04, 5: 1.10); 8 spills into the Newton loop (1.45 ms)
 #endif
 __global__ void __launch_bounds__(128, QK_EX_MINB) exchange_kernel(Geom g, ExchangeConsts kc, double dt, const double *__restrict__ rho,
                                                        double *__restrict__ mx, double *__restrict__ my,
