@@ -42,7 +42,7 @@ namespace qk {
 #define QK_SW_XROWS 4
 #endif
 #ifndef QK_SW_XMINB
-#define QK_SW_XMINB 1
+#define QK_SW_XMINB 5
 #endif
 constexpr int SW_NT = QK_SW_NT;       // threads per CTA of the marching kernels (lanes along x)
 constexpr int SW_NR = 5;              // variables per cell kept in the marching window
