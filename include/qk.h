@@ -130,7 +130,9 @@ int qk_set_params(qk_ctx *ctx, double cfl, double newton_tol, int newton_maxit, 
 int qk_set_state(qk_ctx *ctx, int field, const double *interior);
 int qk_get_state(qk_ctx *ctx, int field, double *interior);
 
-/* Same with the ghost zones: (nz+8)(ny+8)(nx+8) doubles (boundary-fill parity checks). */
+/* Same with the ghost zones: (nz+8)(ny+8)(nx+8) doubles (boundary-fill parity checks, Dirichlet values).  The
+ * step functions fill the ghost zones of their internal reconstruction variables, not necessarily those of the
+ * state fields: call qk_fill_boundary first to see the boundary images of the current state. */
 int qk_set_raw(qk_ctx *ctx, int field, const double *with_ghosts);
 int qk_get_raw(qk_ctx *ctx, int field, double *with_ghosts);
 
