@@ -22,7 +22,7 @@ NG = 4
 FIELDS = ["rho", "mx", "my", "mz", "E", "Er", "Fx", "Fy", "Fz", "kappaP", "kappaR", "src"]
 BC_PERIODIC, BC_OUTFLOW, BC_REFLECTING, BC_FIXED = 0, 1, 2, 3
 FLAG_TAU_CORR, FLAG_STATIC_MATTER, FLAG_NEWTON_LITERAL = 1, 2, 4
-FLAG_PLM, FLAG_EDDINGTON = 8, 16
+FLAG_PLM, FLAG_EDDINGTON, FLAG_MINERBO = 8, 16, 32
 EOS_IDEAL, EOS_ALPHA_T3 = 0, 1
 FILL_HYDRO, FILL_RAD, FILL_ALL = 1, 2, 7
 
@@ -80,6 +80,7 @@ def lib():
         "orc_flatten_1d": (d, [d, dp, dp]),
         "orc_hllc": (None, [d, dp, dp, dp]),
         "orc_eddington_factor": (d, [d]),
+        "orc_minerbo_factor": (d, [d]),
         "orc_closure": (None, [dp, i, dp, dp]),
         "orc_rad_phys_flux": (None, [d, d, dp, i, dp, dp]),
         "orc_rad_hll": (i, [d, d, dp, dp, i, d, u, dp]),

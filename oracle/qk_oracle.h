@@ -45,7 +45,9 @@ enum { ORC_BC_PERIODIC = 0, ORC_BC_OUTFLOW = 1,
                                     PAPER.md:492, 518, 528; inflow boundaries 422, 464, 476 (B2) */  /* solid wall: mirror image, normal momentum / flux component negated */
 enum { ORC_FLAG_TAU_CORR = 1, ORC_FLAG_STATIC_MATTER = 2, ORC_FLAG_NEWTON_LITERAL = 4,
        ORC_FLAG_PLM = 8,          /* piecewise-linear reconstruction with the MC limiter */
-       ORC_FLAG_EDDINGTON = 16 }; /* Eddington approximation chi = 1/3 (P_r = E_r/3)  */
+       ORC_FLAG_EDDINGTON = 16,   /* Eddington approximation chi = 1/3 (P_r = E_r/3)  */
+       ORC_FLAG_MINERBO = 32 };   /* Minerbo (1978) closure in its usual polynomial form
+                                     chi = 1/3 + (2/15) f^2 (3 - f + 3 f^2); NOT printed in PAPER.md (V3) */
 enum { ORC_EOS_IDEAL = 0, ORC_EOS_ALPHA_T3 = 1 };   /* eq 55, PAPER.md:424 (oracle only) */
 enum { ORC_FILL_HYDRO = 1, ORC_FILL_RAD = 2, ORC_FILL_ALL = 7 }; /* bit 4: opacities */
 
@@ -104,6 +106,7 @@ double orc_mc_slope(double qm1, double q0, double qp1);
 double orc_flatten_1d(double gamma, const double P[5], const double vn[5]);
 void   orc_hllc(double gamma, const double WL[5], const double WR[5], double F[5]);
 double orc_eddington_factor(double f);
+double orc_minerbo_factor(double f);
 void   orc_closure(const double fvec[3], int n, double T_col[3], double *chi_out);
 void   orc_closure_k(unsigned flags, const double fvec[3], int n, double T_col[3], double *chi_out);
 void   orc_rad_phys_flux(double c, double c_hat, const double S[4], int n, double G[4], double *Tnn);

@@ -35,6 +35,14 @@ void orc_closure(const double fvec[3], int n, double T_col[3], double *chi_out)
     if (chi_out) *chi_out = chi;
 }
 
+/* Minerbo (1978) maximum-entropy closure in the polynomial form used throughout the transport literature
+ * (PAPER.md:196 names the closure, prints no formula; V3): chi(0) = 1/3, chi(1) = 1. */
+double orc_minerbo_factor(double f)
+{
+    double f2 = f * f;
+    return 1.0 / 3.0 + (2.0 / 15.0) * (f2 * ((3.0 - f) + 3.0 * f2));
+}
+
 /* closure selected by the flags: Levermore (eq 23-25, default) or the Eddington approximation chi = 1/3,
  * i.e. P_r = E_r/3 I whatever the flux ("any local closure f -> chi") */
 void orc_closure_k(unsigned flags, const double fvec[3], int n, double T_col[3], double *chi_out)
@@ -43,6 +51,19 @@ void orc_closure_k(unsigned flags, const double fvec[3], int n, double T_col[3],
         double chi = 1.0 / 3.0;
         double a = 0.5 * (1.0 - chi);
         for (int i = 0; i < 3; ++i) T_col[i] = (i == n) ? a : 0.0;     /* (3chi-1)/2 = 0: no n n term */
+        if (chi_out) *chi_out = chi;
+        return;
+    }
+    if (flags & ORC_FLAG_MINERBO) {     /* as orc_closure with chi from orc_minerbo_factor */
+        double fsq = (fvec[0] * fvec[0] + fvec[1] * fvec[1]) + fvec[2] * fvec[2];
+        double fmag = sqrt(fsq);
+        double chi = orc_minerbo_factor(min2(fmag, 1.0));
+        double a = 0.5 * (1.0 - chi), b = 0.5 * (3.0 * chi - 1.0);
+        for (int i = 0; i < 3; ++i) T_col[i] = (i == n) ? a : 0.0;
+        if (fmag > 0.0) {
+            double nh[3] = { fvec[0] / fmag, fvec[1] / fmag, fvec[2] / fmag };
+            for (int i = 0; i < 3; ++i) T_col[i] = T_col[i] + b * (nh[i] * nh[n]);
+        }
         if (chi_out) *chi_out = chi;
         return;
     }

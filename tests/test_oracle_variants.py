@@ -158,3 +158,32 @@ def test_eddington_linear_wave_speed():
     err = np.abs(g.get_state(5).ravel() - E0).mean() / A
     g.close()
     assert err < 2e-2, err      # back in phase after exactly one period of a c_hat/sqrt(3) wave
+
+
+def test_minerbo_closure_against_its_maximum_entropy_definition():
+    """Minerbo (1978): the Eddington factor of the maximum-entropy intensity I(mu) ~ exp(a mu), i.e.
+    f = coth a - 1/a and chi = 1 - 2 f / a.  The oracle uses the customary polynomial form (PAPER.md:196 prints
+    none, V3); it must hit the limits exactly, be monotone and realizable (f^2 <= chi <= 1) and follow
+    the exact relation closely."""
+    L = O.lib()
+    assert L.orc_minerbo_factor(0.0) == 1.0 / 3.0 and abs(L.orc_minerbo_factor(1.0) - 1.0) < 1e-15
+    fs = np.linspace(0.0, 1.0, 401)
+    chi = np.array([L.orc_minerbo_factor(float(f)) for f in fs])
+    assert np.all(np.diff(chi) > 0) and np.all(chi >= fs ** 2 - 1e-15) and np.all(chi <= 1 + 1e-15)
+    worst = 0.0
+    for f, c in zip(fs[1:-1], chi[1:-1]):
+        lo, hi = 1e-8, 1e4
+        for _ in range(200):                                   # invert the Langevin function by bisection
+            a = 0.5 * (lo + hi)
+            if 1.0 / np.tanh(a) - 1.0 / a < f:
+                lo = a
+            else:
+                hi = a
+        a = 0.5 * (lo + hi)
+        worst = max(worst, abs(c - (1.0 - 2.0 * f / a)))
+    assert worst < 0.011, worst
+    # the closure is selected by its flag and differs from Levermore's in between
+    T, ch = np.zeros(3), np.zeros(1)
+    L.orc_closure_k(O.FLAG_MINERBO, np.array([0.3, 0.4, 0.0]), 0, T, ch)
+    assert ch[0] == L.orc_minerbo_factor(0.5) and abs(ch[0] - L.orc_eddington_factor(0.5)) > 0.02
+    assert abs(T[0] - (0.5 * (1 - ch[0]) + 0.5 * (3 * ch[0] - 1) * 0.36)) < 1e-15
