@@ -54,8 +54,10 @@ enum { QK_FLAG_TAU_CORR = 1,        /* guarded optical-depth correction of the E
        /* scheme variants (sweep path only; QK_EINVAL from the step calls on the cross-check paths): */
        QK_FLAG_PLM = 8,             /* piecewise-linear reconstruction, monotonized-central limiter, for hydro
                                        and radiation instead of PPM                              */
-       QK_FLAG_EDDINGTON = 16 };    /* Eddington approximation chi = 1/3, P_r = E_r/3,
+       QK_FLAG_EDDINGTON = 16,      /* Eddington approximation chi = 1/3, P_r = E_r/3,
                                        instead of the Levermore closure                                         */
+       QK_FLAG_MINERBO = 32 };      /* Minerbo (1978) closure, chi = 1/3 + (2/15) f^2 (3 - f + 3 f^2) (
+                                       formula from the literature, V3); not together with QK_FLAG_EDDINGTON    */
 
 enum { QK_FILL_HYDRO = 1, QK_FILL_RAD = 2, QK_FILL_OPACITY = 4, QK_FILL_ALL = 7 };
 

@@ -19,7 +19,7 @@ FIELDS = ["rho", "mx", "my", "mz", "E", "Er", "Fx", "Fy", "Fz", "kappaP", "kappa
 QK_OK, QK_EINVAL, QK_ENOMEM, QK_ECUDA, QK_ENEWTON, QK_ESTATE = range(6)
 QK_BC_PERIODIC, QK_BC_OUTFLOW, QK_BC_REFLECTING, QK_BC_FIXED = 0, 1, 2, 3
 QK_FLAG_TAU_CORR, QK_FLAG_STATIC_MATTER, QK_FLAG_NEWTON_LITERAL = 1, 2, 4
-QK_FLAG_PLM, QK_FLAG_EDDINGTON = 8, 16
+QK_FLAG_PLM, QK_FLAG_EDDINGTON, QK_FLAG_MINERBO = 8, 16, 32
 QK_FILL_HYDRO, QK_FILL_RAD, QK_FILL_OPACITY, QK_FILL_ALL = 1, 2, 4, 7
 QK_PATH_FUSED, QK_PATH_UNFUSED, QK_PATH_SWEEP = 0, 1, 2
 

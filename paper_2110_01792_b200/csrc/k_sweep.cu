@@ -358,9 +358,10 @@ int launch_rad_sweeps(const Geom &g, const PhysConsts &pc, double dtdx, int stag
         ph.c = pc.c; ph.c_hat = pc.c_hat; ph.dx = pc.dx; ph.tau_corr = (pc.flags & QK_FLAG_TAU_CORR) ? 1 : 0;
         return launch_sweeps(ph, g, dtdx, stage, d, u, u0, o, so, ctr, nullptr, st, which);
     };
-    const bool plm = (pc.flags & QK_FLAG_PLM) != 0, edd = (pc.flags & QK_FLAG_EDDINGTON) != 0;
-    if (plm) return edd ? go(RadPhT<1, 1>()) : go(RadPhT<1, 0>());
-    return edd ? go(RadPhT<0, 1>()) : go(RadPhT<0, 0>());
+    const bool plm = (pc.flags & QK_FLAG_PLM) != 0;
+    const int cl = (pc.flags & QK_FLAG_EDDINGTON) ? 1 : ((pc.flags & QK_FLAG_MINERBO) ? 2 : 0);
+    if (plm) return cl == 1 ? go(RadPhT<1, 1>()) : (cl == 2 ? go(RadPhT<1, 2>()) : go(RadPhT<1, 0>()));
+    return cl == 1 ? go(RadPhT<0, 1>()) : (cl == 2 ? go(RadPhT<0, 2>()) : go(RadPhT<0, 0>()));
 }
 
 }  // namespace qk

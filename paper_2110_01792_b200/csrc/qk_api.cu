@@ -258,7 +258,7 @@ void hydro_stage(qk_ctx *c, double dtdx, int stage, double *const *U, double *co
 // the PLM / Eddington variants and Dirichlet faces exist in the sweep path only
 bool scheme_supported(const qk_ctx *c)
 {
-    return c->path == QK_PATH_SWEEP || (!(c->pc.flags & (QK_FLAG_PLM | QK_FLAG_EDDINGTON)) && !c->has_fixed);
+    return c->path == QK_PATH_SWEEP || (!(c->pc.flags & (QK_FLAG_PLM | QK_FLAG_EDDINGTON | QK_FLAG_MINERBO)) && !c->has_fixed);
 }
 
 int do_hydro_step(qk_ctx *c, double dt, const double *dtdx_dev = nullptr)
@@ -496,6 +496,7 @@ int qk_set_eos(qk_ctx *c, int eos, double alpha)
 int qk_set_params(qk_ctx *c, double cfl, double newton_tol, int newton_maxit, int nsub_max, unsigned flags)
 {
     if (!c || !(cfl > 0.0) || !(newton_tol > 0.0) || newton_maxit < 1 || nsub_max < 1) return QK_EINVAL;
+    if ((flags & QK_FLAG_EDDINGTON) && (flags & QK_FLAG_MINERBO)) return QK_EINVAL;
     c->pc.cfl = cfl; c->pc.newton_tol = newton_tol; c->pc.newton_maxit = newton_maxit;
     c->pc.nsub_max = nsub_max; c->pc.flags = flags;
     return QK_OK;

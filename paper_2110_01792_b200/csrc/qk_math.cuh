@@ -193,20 +193,28 @@ QK_HD double eddington_factor(double f)
     return (3.0 + 4.0 * f2) / (5.0 + 2.0 * sqrt(4.0 - 3.0 * f2));
 }
 
+// Minerbo (1978) closure in its customary polynomial form (V3): chi(0) = 1/3, chi(1) = 1.
+QK_HD double minerbo_factor(double f)
+{
+    const double f2 = f * f;
+    return 1.0 / 3.0 + (2.0 / 15.0) * (f2 * ((3.0 - f) + 3.0 * f2));
+}
+
 // Physical flux of the face state (E, f_x, f_y, f_z) through a face with normal n (0,1,2):
 // (c_hat/c) F_n for E_r and c c_hat E_r T_in for F_i (eq 11-12), with
 // T = (1-chi)/2 I + (3chi-1)/2 n n (eq 23), |f| clamped to 1 for the closure only (R4),
 // n = f/|f| (eq 25), isotropic when f = 0.  Returns T_nn in Tnn.
 struct Rad4 { double e, x, y, z; };
 
-// CL = closure: 0 Levermore (eq 24), 1 Eddington approximation chi = 1/3 (the n n term vanishes)
+// CL = closure: 0 Levermore (eq 24), 1 Eddington approximation chi = 1/3 (the n n term vanishes),
+// 2 Minerbo
 template <int CL = 0>
 QK_HD Rad4 rad_physical_flux(double c, double c_hat, double E, double fx, double fy, double fz, int n,
                              double &Tnn)
 {
     const double fsq = (fx * fx + fy * fy) + fz * fz;
     const double fmag = CL == 1 ? 0.0 : sqrt(fsq);
-    const double chi = CL == 1 ? 1.0 / 3.0 : eddington_factor(lesser(fmag, 1.0));
+    const double chi = CL == 1 ? 1.0 / 3.0 : (CL == 2 ? minerbo_factor(lesser(fmag, 1.0)) : eddington_factor(lesser(fmag, 1.0)));
     const double iso = 0.5 * (1.0 - chi), aniso = 0.5 * (3.0 * chi - 1.0);
     double Tx = (n == 0) ? iso : 0.0, Ty = (n == 1) ? iso : 0.0, Tz = (n == 2) ? iso : 0.0;
     if (fmag > 0.0) {

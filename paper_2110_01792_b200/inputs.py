@@ -14,7 +14,7 @@ import numpy as np
 FIELDS = ["rho", "mx", "my", "mz", "E", "Er", "Fx", "Fy", "Fz", "kappaP", "kappaR"]
 BC_PERIODIC, BC_OUTFLOW, BC_REFLECTING, BC_FIXED = 0, 1, 2, 3
 FLAG_TAU_CORR, FLAG_STATIC_MATTER, FLAG_NEWTON_LITERAL = 1, 2, 4
-FLAG_PLM, FLAG_EDDINGTON = 8, 16     # scheme variants
+FLAG_PLM, FLAG_EDDINGTON, FLAG_MINERBO = 8, 16, 32     # scheme variants
 
 
 def _rng(seed):

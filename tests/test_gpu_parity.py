@@ -287,8 +287,9 @@ def test_hydro_plm_ragged_shocks(bc):
     assert not np.array_equal(ppm[1][1]["rho"], res[1][1]["rho"])
 
 
-@pytest.mark.parametrize("variant", [I.FLAG_PLM, I.FLAG_EDDINGTON, I.FLAG_PLM | I.FLAG_EDDINGTON],
-                         ids=["plm", "eddington", "plm+eddington"])
+@pytest.mark.parametrize("variant", [I.FLAG_PLM, I.FLAG_EDDINGTON, I.FLAG_PLM | I.FLAG_EDDINGTON, I.FLAG_MINERBO,
+                                     I.FLAG_PLM | I.FLAG_MINERBO],
+                         ids=["plm", "eddington", "plm+eddington", "minerbo", "plm+minerbo"])
 def test_rad_transport_variants_config3_small(variant):
     params, fields = I.config3(shape=(24, 20, 28))
     params["flags"] |= variant
