@@ -57,6 +57,7 @@ def lib():
         "orc_set_constants": (None, [p, d, d]),
         "orc_set_params": (None, [p, d, d, i, i, u]),
         "orc_set_eos": (None, [p, i, d]),
+        "orc_set_opacity_law": (None, [p, d, d, d, i]),
         "orc_set_face_bc": (i, [p, np.ctypeslib.ndpointer(dtype=np.int32, flags="C_CONTIGUOUS")]),
         "orc_set_field": (None, [p, i, dp]),
         "orc_get_field": (None, [p, i, dp]),
@@ -121,6 +122,9 @@ class Grid:
 
     def set_params(self, cfl=0.3, newton_tol=1e-10, newton_maxit=400, nsub_max=10, flags=FLAG_TAU_CORR):
         self.L.orc_set_params(self.h, cfl, newton_tol, newton_maxit, nsub_max, flags)
+
+    def set_opacity_law(self, kP0, kR0, rho0, exponent):
+        self.L.orc_set_opacity_law(self.h, kP0, kR0, rho0, exponent)
 
     def set_face_bc(self, bc6):
         """Per-face boundary types (x-lo, x-hi, y-lo, y-hi, z-lo, z-hi)."""

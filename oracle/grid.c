@@ -56,6 +56,14 @@ void orc_set_params(orc_grid *g, double cfl, double newton_tol, int newton_maxit
 
 void orc_set_eos(orc_grid *g, int eos, double alpha) { g->eos = eos; g->alpha = alpha; }
 
+/* Density power-law opacities of the paper's tests: kappa = kappa0 (rho/rho0)^e with integer e
+ * (rho kappa ~ rho^2, e = 1; kappa ~ 1/rho, e = -1).  rho0 = 0 switches the law off
+ * (opacities are then the fields the caller set).  DESIGN.md X14. */
+void orc_set_opacity_law(orc_grid *g, double kP0, double kR0, double rho0, int exponent)
+{
+    g->opac_kP0 = kP0; g->opac_kR0 = kR0; g->opac_rho0 = rho0; g->opac_exp = exponent;
+}
+
 void orc_set_field(orc_grid *g, int field, const double *interior)
 {
     for (int k = 0; k < g->nz; ++k)

@@ -60,6 +60,7 @@ typedef struct orc_grid {
     double cfl, newton_tol;
     int newton_maxit, nsub_max;
     unsigned flags;
+    int opac_exp; double opac_kP0, opac_kR0, opac_rho0;   /* opacity law (orc_set_opacity_law), opac_rho0 = 0: fields */
     int eos; double alpha;          /* ORC_EOS_ALPHA_T3: E_g = alpha T^4 / 4           */
     double S_src;                   /* S of eq 27 for the cell orc_exchange_cell is called on; orc_exchange sets it
                                        to dt * f[ORC_SRC][cell] (0 in every BASELINE config)                  */
@@ -80,6 +81,7 @@ long long orc_ncells_total(const orc_grid *g);
 void   orc_set_constants(orc_grid *g, double a_rad, double kB_mu);
 void   orc_set_params(orc_grid *g, double cfl, double newton_tol, int newton_maxit, int nsub_max, unsigned flags);
 void   orc_set_eos(orc_grid *g, int eos, double alpha);
+void   orc_set_opacity_law(orc_grid *g, double kP0, double kR0, double rho0, int exponent);
 int    orc_set_face_bc(orc_grid *g, const int bc6[6]);   /* 0 ok, 1 if periodic is not on both faces of an axis */
 void   orc_set_field(orc_grid *g, int field, const double *interior);
 void   orc_get_field(const orc_grid *g, int field, double *interior);

@@ -216,9 +216,28 @@ static int rad_divergence(orc_grid *g, double *const R[4], double *div[4])
     return rc;
 }
 
+/* kappa = kappa0 q^|e| with q = rho/rho0 (e > 0) or rho0/rho (e < 0), by repeated multiplication, for the
+ * interior cells, from the density the hydro step left (opacities are static during a radiation subcycle) */
+static void apply_opacity_law(orc_grid *g)
+{
+    if (!(g->opac_rho0 > 0.0)) return;
+    const int n = g->opac_exp < 0 ? -g->opac_exp : g->opac_exp;
+    for (int k = 0; k < g->nz; ++k)
+        for (int j = 0; j < g->ny; ++j)
+            for (int i = 0; i < g->nx; ++i) {
+                long long c = ((long long)(k + NG) * (g->ny + 2 * NG) + (j + NG)) * (g->nx + 2 * NG) + (i + NG);
+                double rho = g->f[ORC_RHO][c];
+                double q = g->opac_exp < 0 ? g->opac_rho0 / rho : rho / g->opac_rho0;
+                double kp = g->opac_kP0, kr = g->opac_kR0;
+                for (int m = 0; m < n; ++m) { kp = kp * q; kr = kr * q; }
+                g->f[ORC_KP][c] = kp; g->f[ORC_KR][c] = kr;
+            }
+}
+
 /* one radiation subcycle of transport: the same SSP-RK2 as hydro */
 int orc_rad_transport(orc_grid *g, double dt)
 {
+    apply_opacity_law(g);
     const long long ntot = orc_ncells_total(g);
     const int nx = g->nx, ny = g->ny, nz = g->nz;
     double *div[4], *R0[4], *R[4];

@@ -132,3 +132,36 @@ def test_beam_entering_through_a_fixed_face_streams_at_c_hat():
     half = x[np.nonzero(E > 0.5)[0][-1]]
     assert abs(half - front) < 0.03
     g.close()
+
+
+def test_density_power_law_opacities():
+    """kappa = kappa0 (rho/rho0)^e (PAPER.md:464 e = 1, PAPER.md:528 e = -1).  With e = -1 the extinction rho kappa is
+    the same everywhere whatever the density field, so the radiation evolves as in a uniform medium of the same
+    rho kappa; with e = 1 in a uniform medium of density 2 rho0 the law is the constant field 2 kappa0, bit for bit."""
+    N, c, c_hat = 64, 1.0, 0.5
+    x = (np.arange(N) + 0.5) / N
+    E0 = 1.0 + np.exp(-((x - 0.5) / 0.08) ** 2)
+
+    def run(rho, law=None, kfield=None, nsteps=40):
+        g = O.Grid(N, 1, 1, 1.0 / N, G53, c_hat=c_hat, c=c)
+        g.set_params(flags=O.FLAG_STATIC_MATTER | O.FLAG_TAU_CORR)
+        for name, a in (("rho", rho), ("E", 1.5 * rho), ("Er", E0)):
+            g.set_state(O.FIELDS.index(name), a.reshape(1, 1, N))
+        if law:
+            g.set_opacity_law(*law)
+        else:
+            g.set_state(O.FIELDS.index("kappaR"), np.full((1, 1, N), kfield))
+        for _ in range(nsteps):
+            assert g.rad_step(0.3 / N / c_hat) == 0
+        out = g.get_state(5).ravel(), g.get_state(10).ravel()
+        g.close()
+        return out
+
+    wavy = 1.0 + 0.5 * np.sin(2 * np.pi * x)
+    Er_law, kR = run(wavy, law=(0.0, 50.0, 1.0, -1))
+    assert np.abs(kR * wavy - 50.0).max() < 1e-13 * 50
+    Er_uni, _ = run(np.ones(N), kfield=50.0)
+    assert np.abs(Er_law - Er_uni).max() < 1e-12 and np.abs(Er_uni - E0).max() > 0.05
+    Er_a, kR_a = run(np.full(N, 2.0), law=(0.0, 50.0, 1.0, 1))
+    Er_b, _ = run(np.full(N, 2.0), kfield=100.0)
+    assert np.all(kR_a == 100.0) and np.array_equal(Er_a, Er_b)
