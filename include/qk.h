@@ -115,6 +115,12 @@ int qk_set_constants(qk_ctx *ctx, double a_rad, double kB_over_mu_mH);
  * (all state fields, the whole ghost slab including edges and corners) with qk_set_raw before stepping. */
 int qk_set_face_boundaries(qk_ctx *ctx, const int *bc6);
 
+/* Density power-law opacities kappa_P,R = kappa0_P,R (rho/rho0)^exponent, integer exponent in [-4, 4] (the laws of
+ * the paper's tests: rho kappa ~ rho^2; kappa ~ 1/rho; X14).  When rho0 > 0 the two
+ * opacity fields of the interior cells are recomputed from the current density at the start of every radiation
+ * subcycle; rho0 = 0 (default) leaves the fields as the caller set them. */
+int qk_set_opacity_law(qk_ctx *ctx, double kappaP0, double kappaR0, double rho0, int exponent);
+
 /* Equation of state of the gas in the EXCHANGE step: QK_EOS_IDEAL (default; T = (gamma-1) E_g / (rho k_B/(mu m_H)))
  * or QK_EOS_ALPHA_T3, E_g = alpha T^4 / 4 with volumetric heat capacity C_v = alpha T^3 (eq 55, PAPER.md:424-427;
  * the Marshak, Su-Olson and energy-exchange tests, where the matter is static).  The hydro step always uses the

@@ -29,7 +29,7 @@ EXPORTS = [
     "qk_cfl_dt", "qk_hydro_step", "qk_rad_transport", "qk_exchange", "qk_rad_step", "qk_rhd_step",
     "qk_nsub_for", "qk_last_info", "qk_launch_count", "qk_set_path", "qk_set_profiling",
     "qk_kernel_class_count", "qk_kernel_class_name", "qk_kernel_times", "qk_version", "qk_fp64_probe",
-    "qk_selftest_divsqrt", "qk_set_eos", "qk_set_face_boundaries", "qk_hydro_step_cfl", "qk_last_dt", "qk_set_halo_exchange", "qk_halo_doubles", "qk_halo_pack", "qk_halo_unpack",
+    "qk_selftest_divsqrt", "qk_set_eos", "qk_set_opacity_law", "qk_set_face_boundaries", "qk_hydro_step_cfl", "qk_last_dt", "qk_set_halo_exchange", "qk_halo_doubles", "qk_halo_pack", "qk_halo_unpack",
 ]
 
 
@@ -70,6 +70,7 @@ def lib():
         "qk_set_constants": (i, [p, d, d]),
         "qk_set_params": (i, [p, d, d, i, i, u]),
         "qk_set_eos": (i, [p, i, d]),
+        "qk_set_opacity_law": (i, [p, d, d, d, i]),
         "qk_set_face_boundaries": (i, [p, C.POINTER(C.c_int)]),
         "qk_set_state": (i, [p, i, p]),
         "qk_get_state": (i, [p, i, p]),
@@ -196,6 +197,9 @@ class Context:
     def qk_set_face_boundaries(self, bc6):
         arr = (C.c_int * 6)(*[int(b) for b in bc6])
         _check(self.L.qk_set_face_boundaries(self.h, arr), "qk_set_face_boundaries")
+
+    def qk_set_opacity_law(self, kappaP0, kappaR0, rho0, exponent):
+        _check(self.L.qk_set_opacity_law(self.h, kappaP0, kappaR0, rho0, exponent), "qk_set_opacity_law")
 
     def qk_set_eos(self, eos, alpha=0.0):
         _check(self.L.qk_set_eos(self.h, eos, alpha), "qk_set_eos")

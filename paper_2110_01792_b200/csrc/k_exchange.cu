@@ -73,6 +73,30 @@ __global__ void __launch_bounds__(128, QK_EX_MINB) exchange_kernel(Geom g, Excha
     }
 }
 
+// kappa = kappa0 q^|e|, q = rho/rho0 (e > 0) or rho0/rho (e < 0), by repeated multiplication (X14): the density
+// power laws of the paper's tests, interior cells, evaluated before a radiation subcycle
+__global__ void __launch_bounds__(128) opacity_law_kernel(Geom g, const double *__restrict__ rho, double *__restrict__ kP,
+                                                          double *__restrict__ kR, double kP0, double kR0, double rho0, int e)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= g.nx) return;
+    const int cidx = g.at(i, blockIdx.y, blockIdx.z);
+    const double r = rho[cidx];
+    const double q = e < 0 ? rho0 / r : r / rho0;
+    const int n = e < 0 ? -e : e;
+    double kp = kP0, kr = kR0;
+    for (int m = 0; m < n; ++m) { kp = kp * q; kr = kr * q; }
+    kP[cidx] = kp; kR[cidx] = kr;
+}
+
+int launch_opacity_law(const Geom &g, const double *rho, double *kP, double *kR, double kP0, double kR0, double rho0,
+                       int e, cudaStream_t st)
+{
+    dim3 grid((g.nx + 127) / 128, g.ny, g.nz);
+    opacity_law_kernel<<<grid, 128, 0, st>>>(g, rho, kP, kR, kP0, kR0, rho0, e);
+    return 1;
+}
+
 int launch_exchange(const Geom &g, const PhysConsts &pc, double dt, const double *rho, double *mx, double *my,
                     double *mz, double *E, double *Er, double *Fx, double *Fy, double *Fz, const double *kP,
                     const double *kR, const double *src, Hydro5 Wout, Rad4p Sout, Counters *ctr, StateCache *cache,

@@ -347,6 +347,11 @@ void rad_stage(qk_ctx *c, double dtdx, int stage, double *const *R, double *cons
 int do_rad_transport(qk_ctx *c, double dt)
 {
     if (!scheme_supported(c)) return QK_EINVAL;
+    if (c->pc.opac_rho0 > 0.0) {         // opacities follow the density the hydro step left (X14)
+        Scope s(c, K_RAD_PRIM);
+        s.done(launch_opacity_law(c->g, c->state[QK_RHO], c->state[QK_KAPPA_P], c->state[QK_KAPPA_R], c->pc.opac_kP0,
+                                  c->pc.opac_kR0, c->pc.opac_rho0, c->pc.opac_exp, c->stream));
+    }
     const double dtdx = dt / c->pc.dx;
     double *const *Rn = &c->state[QK_ER];
     double *const *R1 = &c->stage[0];
@@ -421,7 +426,8 @@ int qk_init(int nx, int ny, int nz, double dx, double gamma, double c_hat, doubl
     if (!x) return QK_ENOMEM;
     x->g = make_geom(nx, ny, nz);
     x->pc.dx = dx; x->pc.gamma = gamma; x->pc.c_hat = c_hat; x->pc.c = c;
-    x->pc.a_rad = 1.0; x->pc.kB_mu = 1.0; x->pc.eos_alpha = 0.0; x->pc.cfl = 0.3; x->pc.newton_tol = 1e-10;
+    x->pc.a_rad = 1.0; x->pc.kB_mu = 1.0; x->pc.eos_alpha = 0.0;
+    x->pc.opac_kP0 = 0.0; x->pc.opac_kR0 = 0.0; x->pc.opac_rho0 = 0.0; x->pc.opac_exp = 0; x->pc.cfl = 0.3; x->pc.newton_tol = 1e-10;
     x->pc.newton_maxit = 400; x->pc.nsub_max = 10; x->pc.flags = QK_FLAG_TAU_CORR; x->pc.bc = boundary;
     x->stream = nullptr; x->device = dev; x->base = nullptr; x->bytes = 0; x->owns = false; x->ready = false;
     x->path = QK_PATH_SWEEP; x->w_cur = 0; x->s_cur = 0; x->w_valid = false; x->s_valid = false; x->smax_valid = false; x->has_source = false; x->has_fixed = boundary == QK_BC_FIXED;
@@ -483,6 +489,13 @@ int qk_set_face_boundaries(qk_ctx *c, const int *bc6)
     c->has_fixed = false;
     for (int f = 0; f < 6; ++f) { c->fb.t[f] = bc6[f]; c->has_fixed = c->has_fixed || bc6[f] == QK_BC_FIXED; }
     c->w_valid = false; c->s_valid = false;
+    return QK_OK;
+}
+
+int qk_set_opacity_law(qk_ctx *c, double kappaP0, double kappaR0, double rho0, int exponent)
+{
+    if (!c || !(kappaP0 >= 0.0) || !(kappaR0 >= 0.0) || !(rho0 >= 0.0) || exponent < -4 || exponent > 4) return QK_EINVAL;
+    c->pc.opac_kP0 = kappaP0; c->pc.opac_kR0 = kappaR0; c->pc.opac_rho0 = rho0; c->pc.opac_exp = exponent;
     return QK_OK;
 }
 

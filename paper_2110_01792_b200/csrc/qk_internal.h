@@ -65,6 +65,8 @@ enum KClass { K_FILL = 0, K_CFL, K_PRIM, K_FLATTEN, K_HYDRO_FLUX, K_HYDRO_UPDATE
 
 struct PhysConsts {
     double dx, gamma, c_hat, c, a_rad, kB_mu, cfl, newton_tol;
+    double opac_kP0, opac_kR0, opac_rho0;   // opacity law (qk_set_opacity_law); opac_rho0 = 0: the fields as set
+    int opac_exp;
     double eos_alpha;      // > 0: E_g = alpha T^4 / 4 in the exchange (eq 55); 0: ideal gas
     int newton_maxit, nsub_max;
     unsigned flags;
@@ -117,6 +119,8 @@ int launch_rad_flux(const Geom &g, const PhysConsts &pc, int dir, CRad4p S, cons
 int launch_rad_update(const Geom &g, double dtdx, int stage, CRad4p R, CRad4p R0, CRad4p gx, CRad4p gy, CRad4p gz,
                       Rad4p out, cudaStream_t st);
 
+int launch_opacity_law(const Geom &g, const double *rho, double *kP, double *kR, double kP0, double kR0, double rho0,
+                       int e, cudaStream_t st);
 int launch_exchange(const Geom &g, const PhysConsts &pc, double dt, const double *rho, double *mx, double *my,
                     double *mz, double *E, double *Er, double *Fx, double *Fy, double *Fz, const double *kP,
                     const double *kR, const double *src, Hydro5 Wout, Rad4p Sout, Counters *ctr, StateCache *cache,

@@ -882,3 +882,95 @@ def test_full_size_conservation_config2_and_config4():
     e0 = _sum(fields["E"]) + (c / ch) * _sum(fields["Er"])
     e1 = _sum(got["E"]) + (c / ch) * _sum(got["Er"])
     assert abs(e1 - e0) < 1e-12 * e0
+
+
+# ------------------------------------------------------------------------------------------------
+# the subcritical radiative shock (Lowrie & Edwards Mach 3), every printed parameter
+# ------------------------------------------------------------------------------------------------
+def _radiative_shock_setup(N):
+    c, a_r, kB, mH = 2.99792458e10, 7.5657e-15, 1.380649e-16, 1.6726219e-24
+    g, kBmu = 5.0 / 3.0, kB / mH
+    left = dict(rho=5.69, v=5.19e7, T=2.18e6)
+    right = dict(rho=17.1, v=1.73e7, T=7.98e6)
+    chat = 10.0 * (left["v"] + np.sqrt(g * kBmu * left["T"]))        # c_hat = 10 (v_L + c_s,L)
+    Lx, x0 = 0.01575, 0.0130
+    dx = Lx / N
+    xg = (np.arange(-4, N + 4) + 0.5) * dx
+    rho, v, T = (np.where(xg < x0, left[k], right[k]) for k in ("rho", "v", "T"))
+    P = rho * kBmu * T
+    raw = {0: rho, 1: rho * v, 2: 0 * rho, 3: 0 * rho, 4: P / (g - 1) + 0.5 * rho * v * v, 5: a_r * T ** 4,
+           6: 0 * rho, 7: 0 * rho, 8: 0 * rho, 9: 577.0 / rho, 10: 577.0 / rho}
+    raw = {f: np.ascontiguousarray(np.broadcast_to(a, (9, 9, N + 8))) for f, a in raw.items()}
+    return dict(c=c, a_r=a_r, kBmu=kBmu, g=g, chat=chat, dx=dx, Lx=Lx, x0=x0, left=left, right=right, raw=raw)
+
+
+def _radiative_shock_ctx(s, N):
+    ctx = B.Context(N, 1, 1, s["dx"], s["g"], s["chat"], s["c"])
+    ctx.qk_set_constants(s["a_r"], s["kBmu"])
+    ctx.qk_set_params(cfl=0.4, flags=B.QK_FLAG_TAU_CORR | B.QK_FLAG_EDDINGTON)      # P_r = E_r/3
+    ctx.qk_set_face_boundaries([B.QK_BC_FIXED, B.QK_BC_FIXED, 0, 0, 0, 0])           # asymptotic states as Dirichlet
+    ctx.qk_set_opacity_law(577.0, 577.0, 1.0, -1)                                    # kappa = 577 (1 g cm^-3 / rho)
+    for f, a in s["raw"].items():
+        ctx.qk_set_raw(f, a)
+    return ctx
+
+
+def test_gpu_subcritical_radiative_shock():
+    """512 cells on [0, 0.01575] cm, membrane at 0.0130 cm, t = 1e-9 s, CFL 0.4, Eddington closure, c_hat = 10 (v_L +
+    c_s,L).  The paper reports a steady structure whose shock has drifted 1.5 % of the domain to the right; without
+    the semi-analytic profile (not in this container) the checks are the ones a steady radiative shock must pass:
+    uniform mass flux, asymptotic states kept, radiative precursor with T_rad > T_gas ahead of the shock, monotone
+    T_rad, a Zel'dovich spike in T_gas behind it, and that drift."""
+    N = 512
+    s = _radiative_shock_setup(N)
+    with _radiative_shock_ctx(s, N) as ctx:
+        t, tend, nsub_max = 0.0, 1e-9, 0
+        while t < tend * (1 - 1e-12):
+            dt = min(ctx.qk_cfl_dt(), tend - t)
+            ctx.qk_rhd_step(dt)
+            t += dt
+        info = ctx.qk_last_info()
+        U = [ctx.qk_get_state(f).ravel() for f in range(9)]
+    assert info["status"] == 0 and info["nsub"] > 1
+    x = (np.arange(N) + 0.5) * s["dx"]
+    rho, vel = U[0], U[1] / U[0]
+    Tg = (s["g"] - 1) * (U[4] - 0.5 * rho * vel ** 2) / (rho * s["kBmu"])
+    Tr = (U[5] / s["a_r"]) ** 0.25
+    L, R = s["left"], s["right"]
+    mdot = 0.5 * (L["rho"] * L["v"] + R["rho"] * R["v"])
+    assert np.abs(rho * vel / mdot - 1.0).max() < 0.015                       # steady: rho v uniform
+    assert abs(rho[:8].mean() / L["rho"] - 1) < 1e-3 and abs(Tg[:8].mean() / L["T"] - 1) < 1e-3
+    assert abs(rho[-8:].mean() / R["rho"] - 1) < 1e-2 and abs(Tg[-8:].mean() / R["T"] - 1) < 1e-2
+    shock = x[np.abs(np.diff(rho)).argmax()]
+    drift = (shock - s["x0"]) / s["Lx"]
+    assert 0.005 < drift < 0.025, drift                                       # paper: 1.5 per cent to the right
+    ahead = (x > 0.006) & (x < shock - 0.0005)
+    assert np.all(Tr[ahead] > Tg[ahead]) and Tg[ahead].min() > 1.02 * L["T"]  # precursor heated by radiation
+    assert np.diff(Tr).min() > -1e-4 * Tr.max()                               # T_rad continuous and monotone
+    assert 1.05 < Tg.max() / R["T"] < 1.30 and shock - 1e-4 < x[Tg.argmax()] < shock + 6e-4   # Zel'dovich spike
+
+
+def test_radiative_shock_ingredients_parity_with_oracle():
+    """The same setup at 48 cells for 40 steps against the oracle: Dirichlet faces, Eddington closure, kappa ~ 1/rho,
+    subcycled RHD steps in cgs units -- bit for bit."""
+    N = 48
+    s = _radiative_shock_setup(N)
+    g = O.Grid(N, 1, 1, s["dx"], s["g"], c_hat=s["chat"], c=s["c"])
+    g.set_constants(s["a_r"], s["kBmu"])
+    g.set_params(cfl=0.4, flags=O.FLAG_TAU_CORR | O.FLAG_EDDINGTON)
+    g.set_face_bc([O.BC_FIXED, O.BC_FIXED, 0, 0, 0, 0])
+    g.set_opacity_law(577.0, 577.0, 1.0, -1)
+    for f, a in s["raw"].items():
+        g.set_raw(f, a)
+    with _radiative_shock_ctx(s, N) as ctx:
+        nsubs = set()
+        for _ in range(40):
+            dt = g.cfl_dt()
+            assert ctx.qk_cfl_dt() == dt
+            assert g.rhd_step(dt) == 0
+            ctx.qk_rhd_step(dt)
+            nsubs.add(ctx.qk_last_info()["nsub"])
+        for f in range(11):
+            assert np.array_equal(g.get_state(f), ctx.qk_get_state(f)), B.FIELDS[f]
+        assert max(nsubs) > 1 and ctx.qk_last_info()["newton_total_iters"] == g.info()["newton_total_iters"]
+    g.close()
