@@ -22,19 +22,20 @@ NG = 4
 FIELDS = ["rho", "mx", "my", "mz", "E", "Er", "Fx", "Fy", "Fz", "kappaP", "kappaR", "src"]
 BC_PERIODIC, BC_OUTFLOW, BC_REFLECTING, BC_FIXED = 0, 1, 2, 3
 FLAG_TAU_CORR, FLAG_STATIC_MATTER, FLAG_NEWTON_LITERAL = 1, 2, 4
-FLAG_PLM, FLAG_EDDINGTON, FLAG_MINERBO = 8, 16, 32
+FLAG_PLM, FLAG_EDDINGTON, FLAG_MINERBO, FLAG_NO_DKAPPA_DT = 8, 16, 32, 64
 EOS_IDEAL, EOS_ALPHA_T3 = 0, 1
 FILL_HYDRO, FILL_RAD, FILL_ALL = 1, 2, 7
 
 
 def build(force: bool = False) -> str:
-    """gcc -O2 -ffp-contract=off (no FMA contraction) -> libqk_oracle.so"""
+    """gcc -O2 -ffp-contract=off (no FMA contraction) -fopenmp (independent cells dealt out to
+    threads; no result bit depends on the thread count) -> libqk_oracle.so"""
     srcs = [os.path.join(_HERE, s) for s in _SRCS]
     deps = srcs + [os.path.join(_HERE, "qk_oracle.h")]
     if (not force and os.path.exists(_LIB)
             and os.path.getmtime(_LIB) >= max(os.path.getmtime(d) for d in deps)):
         return _LIB
-    cmd = ["gcc", "-O2", "-ffp-contract=off", "-fno-fast-math", "-std=c99", "-shared", "-fPIC",
+    cmd = ["gcc", "-O2", "-ffp-contract=off", "-fno-fast-math", "-std=c99", "-fopenmp", "-shared", "-fPIC",
            "-o", _LIB] + srcs + ["-lm"]
     subprocess.run(cmd, check=True, cwd=_HERE)
     return _LIB
@@ -47,6 +48,9 @@ def lib():
     global _lib
     if _lib is not None:
         return _lib
+    # idle worker threads sleep instead of spinning, so that several processes using the oracle at once (pytest-xdist,
+    # a test next to a bench) do not starve each other; read by libgomp when it is loaded
+    os.environ.setdefault("OMP_WAIT_POLICY", "passive")
     L = C.CDLL(build())
     d, i, p, u = C.c_double, C.c_int, C.c_void_p, C.c_uint
     dp = np.ctypeslib.ndpointer(dtype=np.float64, flags="C_CONTIGUOUS")
@@ -58,6 +62,12 @@ def lib():
         "orc_set_params": (None, [p, d, d, i, i, u]),
         "orc_set_eos": (None, [p, i, d]),
         "orc_set_opacity_law": (None, [p, d, d, d, i]),
+        "orc_set_opacity_law_T": (None, [p, d, d, d, i, d, i]),
+        "orc_set_wavespeed_floor": (None, [p, d]),
+        "orc_set_threads": (None, [i]),
+        "orc_get_threads": (i, []),
+        "orc_rad_hll_floor": (i, [d, d, dp, dp, i, d, u, d, dp]),
+        "orc_temp_power": (d, [d, d, i]),
         "orc_set_face_bc": (i, [p, np.ctypeslib.ndpointer(dtype=np.int32, flags="C_CONTIGUOUS")]),
         "orc_set_field": (None, [p, i, dp]),
         "orc_get_field": (None, [p, i, dp]),
@@ -120,11 +130,18 @@ class Grid:
     def set_constants(self, a_rad, kB_mu):
         self.L.orc_set_constants(self.h, a_rad, kB_mu)
 
-    def set_params(self, cfl=0.3, newton_tol=1e-10, newton_maxit=400, nsub_max=10, flags=FLAG_TAU_CORR):
+    def set_params(self, cfl=0.3, newton_tol=1e-10, newton_maxit=400, nsub_max=10, flags=0):
         self.L.orc_set_params(self.h, cfl, newton_tol, newton_maxit, nsub_max, flags)
 
     def set_opacity_law(self, kP0, kR0, rho0, exponent):
         self.L.orc_set_opacity_law(self.h, kP0, kR0, rho0, exponent)
+
+    def set_opacity_law_T(self, kP0, kR0, rho0, exponent, T0, texp2):
+        """kappa = kappa0 (rho/rho0)^exponent (T/T0)^(texp2/2)"""
+        self.L.orc_set_opacity_law_T(self.h, kP0, kR0, rho0, exponent, T0, texp2)
+
+    def set_wavespeed_floor(self, s_floor):
+        self.L.orc_set_wavespeed_floor(self.h, s_floor)
 
     def set_face_bc(self, bc6):
         """Per-face boundary types (x-lo, x-hi, y-lo, y-hi, z-lo, z-hi)."""
@@ -194,3 +211,12 @@ class Grid:
 
     def nsub_for(self, dt):
         return int(self.L.orc_nsub_for(self.h, dt))
+
+
+def set_threads(n):
+    """worker threads of the oracle's loops over cells (no result depends on it)"""
+    lib().orc_set_threads(int(n))
+
+
+def get_threads():
+    return int(lib().orc_get_threads())

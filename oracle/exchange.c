@@ -24,7 +24,40 @@ static void eos_T_Cv(const orc_grid *g, double rho, double Eg, double *T, double
     }
 }
 
-/* Updates (m, E, Er, F) of one cell over dt.  Returns 0 ok, 4 Newton failure, 5 bad state. */
+/* (T/T0)^(n2/2) for an integer n2 by repeated multiplication, one square root when n2 is odd and one division
+ * when it is negative -- no pow(), so that the CUDA path can reproduce every bit (X14). */
+double orc_temp_power(double T, double T0, int n2)
+{
+    int a = n2 < 0 ? -n2 : n2;
+    double q = T / T0, p = 1.0;
+    for (int m = 0; m < a / 2; ++m) p = p * q;
+    if (a & 1) p = p * sqrt(q);
+    return n2 < 0 ? 1.0 / p : p;
+}
+
+/* density part kappa0 (rho/rho0)^e of the opacity law, integer e by repeated multiplication */
+void orc_opacity_density_part(const orc_grid *g, double rho, double *kP, double *kR)
+{
+    const int n = g->opac_exp < 0 ? -g->opac_exp : g->opac_exp;
+    double q = g->opac_exp < 0 ? g->opac_rho0 / rho : rho / g->opac_rho0;
+    double kp = g->opac_kP0, kr = g->opac_kR0;
+    for (int m = 0; m < n; ++m) { kp = kp * q; kr = kr * q; }
+    *kP = kp; *kR = kr;
+}
+
+/* gas temperature of a cell from its conserved state (PAPER.md:204 and the equation of state) */
+double orc_gas_temperature(const orc_grid *g, double rho, const double m[3], double E)
+{
+    double msq = (m[0] * m[0] + m[1] * m[1]) + m[2] * m[2];
+    double Eg = E - 0.5 * msq / rho, T, Cv;
+    eos_T_Cv(g, rho, Eg, &T, &Cv);
+    return T;
+}
+
+/* Updates (m, E, Er, F) of one cell over dt.  With a temperature-dependent opacity law (orc_set_opacity_law_T,
+ * texp2 != 0) kP and kR are the density parts of the law: kappa_P follows the Newton iterate's temperature and
+ * enters the Jacobian through d kappa_P / dT (eq 33), kappa_F ~ kappa_R is evaluated at the updated
+ * gas temperature.  Returns 0 ok, 4 Newton failure, 5 bad state. */
 int orc_exchange_cell(const orc_grid *g, double dt, double rho, double m[3], double *E,
                       double *Er, double F[3], double kP, double kR, int *iters)
 {
@@ -37,6 +70,7 @@ int orc_exchange_cell(const orc_grid *g, double dt, double rho, double m[3], dou
     double Er0 = *Er;
     double Etot = Eg0 + coc * (Er0 + S);        /* eq 38 */
     double coef = dt * rho * kP * ch;           /* dt rho kappa_P c_hat */
+    const int kT = (g->opac_rho0 > 0.0) && (g->opac_texp2 != 0);   /* kappa(rho, T) law */
     double Eg = Eg0, Erad = Er0;
     int it = 0, done = 0;
     const int literal = (g->flags & ORC_FLAG_NEWTON_LITERAL) != 0;
@@ -45,12 +79,20 @@ int orc_exchange_cell(const orc_grid *g, double dt, double rho, double m[3], dou
         eos_T_Cv(g, rho, Eg, &T, &Cv);
         double T2 = T * T;
         double T4 = T2 * T2;
+        double dcoef_dT = 0.0;
+        if (kT) {                                                 /* kappa_P at the iterate's temperature */
+            double kPT = kP * orc_temp_power(T, g->opac_T0, g->opac_texp2);
+            coef = dt * rho * kPT * ch;
+            double dkP_dT = (0.5 * (double)g->opac_texp2) * kPT / T;
+            if (!(g->flags & ORC_FLAG_NO_DKAPPA_DT)) dcoef_dT = dt * rho * dkP_dT * ch;
+        }
         double R = coef * (g->a_rad * T4 - Erad);                 /* eq 28 (reading X1) */
         double FG = (Eg - Eg0) + coc * R;                         /* eq 26 */
         double FR = (Erad - Er0) - (R + S);                       /* eq 27 */
         int conv = (fabs(FG / Etot) < g->newton_tol) && (fabs(coc * FR / Etot) < g->newton_tol); /* eq 36-37 */
         if (conv && literal) { done = 1; break; }
         double dRdEg = coef * (4.0 * g->a_rad * (T2 * T)) / Cv;   /* eq 33, dkappa/dT = 0 */
+        if (kT) dRdEg = (coef * (4.0 * g->a_rad * (T2 * T)) + dcoef_dT * (g->a_rad * T4 - Erad)) / Cv;   /* eq 33 */
         double dFGdEg = 1.0 + coc * dRdEg;                        /* eq 29 */
         double dFGdEr = -(coc * coef);                            /* eq 30 */
         double dFRdEg = -dRdEg;                                   /* eq 31 */
@@ -66,6 +108,11 @@ int orc_exchange_cell(const orc_grid *g, double dt, double rho, double m[3], dou
     if (!done) rc = 4;                                            /* PAPER.md:247 */
     if (iters) *iters = it;
     /* eq 39-41 with kappa_F ~ kappa_R (PAPER.md:108) */
+    if (kT) {                                                     /* kappa_F at the updated temperature, PAPER.md:249 */
+        double T, Cv;
+        eos_T_Cv(g, rho, Eg, &T, &Cv);
+        kR = kR * orc_temp_power(T, g->opac_T0, g->opac_texp2);
+    }
     double denom = 1.0 + rho * kR * ch * dt;
     double F1[3], m1[3];
     for (int i = 0; i < 3; ++i) F1[i] = F[i] / denom;
@@ -88,7 +135,10 @@ int orc_exchange_cell(const orc_grid *g, double dt, double rho, double m[3], dou
 int orc_exchange(orc_grid *g, double dt)
 {
     const int nx = g->nx, ny = g->ny, nz = g->nz;
+    const long long ntot = orc_ncells_total(g);
+    const int kT = (g->opac_rho0 > 0.0) && (g->opac_texp2 != 0);
     long long fail = 0, tot = 0, bad = 0; int mx = 0;
+#pragma omp parallel for collapse(3) schedule(static) reduction(+ : fail, tot, bad) reduction(max : mx) if (ntot > ORC_OMP_MIN)
     for (int k = 0; k < nz; ++k)
         for (int j = 0; j < ny; ++j)
             for (int i = 0; i < nx; ++i) {
@@ -96,10 +146,12 @@ int orc_exchange(orc_grid *g, double dt)
                 double m[3] = { g->f[ORC_MX][cidx], g->f[ORC_MY][cidx], g->f[ORC_MZ][cidx] };
                 double F[3] = { g->f[ORC_FX][cidx], g->f[ORC_FY][cidx], g->f[ORC_FZ][cidx] };
                 double E = g->f[ORC_E][cidx], Er = g->f[ORC_ER][cidx];
+                double kP = g->f[ORC_KP][cidx], kR = g->f[ORC_KR][cidx];
                 int it = 0;
-                g->S_src = dt * g->f[ORC_SRC][cidx];            /* energy added during the substep (X13) */
-                int r = orc_exchange_cell(g, dt, g->f[ORC_RHO][cidx], m, &E, &Er, F,
-                                          g->f[ORC_KP][cidx], g->f[ORC_KR][cidx], &it);
+                orc_grid cell = *g;                              /* per-cell copy of the parameters: carries S */
+                cell.S_src = dt * g->f[ORC_SRC][cidx];           /* energy added during the substep (X13) */
+                if (kT) orc_opacity_density_part(g, g->f[ORC_RHO][cidx], &kP, &kR);
+                int r = orc_exchange_cell(&cell, dt, g->f[ORC_RHO][cidx], m, &E, &Er, F, kP, kR, &it);
                 if (r == 4) ++fail;
                 if (r == 5) ++bad;
                 tot += it; if (it > mx) mx = it;
@@ -107,7 +159,6 @@ int orc_exchange(orc_grid *g, double dt)
                 g->f[ORC_FX][cidx] = F[0]; g->f[ORC_FY][cidx] = F[1]; g->f[ORC_FZ][cidx] = F[2];
                 g->f[ORC_E][cidx] = E; g->f[ORC_ER][cidx] = Er;
             }
-    g->S_src = 0.0;
     g->newton_fail_cells = fail; g->newton_total_iters = tot; g->newton_max_iters = mx;
     g->bad_state_cells = bad;
     return fail ? 4 : (bad ? 5 : 0);

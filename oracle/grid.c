@@ -29,7 +29,8 @@ orc_grid *orc_create(int nx, int ny, int nz, double dx, double gamma, double c_h
     for (int f = 0; f < 6; ++f) g->face_bc[f] = bc;
     g->a_rad = 1.0; g->kB_mu = 1.0;
     g->cfl = 0.3; g->newton_tol = 1e-10; g->newton_maxit = 400; g->nsub_max = 10; /* PAPER.md:247,273 */
-    g->flags = ORC_FLAG_TAU_CORR;
+    g->flags = 0;                    /* optical-depth correction off: DESIGN.md R6 */
+    g->s_floor = 0.1;                /* wavespeed floor of reading R5, in units of c_hat */
     g->eos = ORC_EOS_IDEAL; g->alpha = 0.0; g->S_src = 0.0;
     long long n = orc_ncells_total(g);
     for (int f = 0; f < ORC_NFIELDS; ++f) {
@@ -62,7 +63,30 @@ void orc_set_eos(orc_grid *g, int eos, double alpha) { g->eos = eos; g->alpha = 
 void orc_set_opacity_law(orc_grid *g, double kP0, double kR0, double rho0, int exponent)
 {
     g->opac_kP0 = kP0; g->opac_kR0 = kR0; g->opac_rho0 = rho0; g->opac_exp = exponent;
+    g->opac_T0 = 1.0; g->opac_texp2 = 0;
 }
+
+/* ... times (T/T0)^(texp2/2), T the gas temperature: half-integer powers such as Kramers' T^-3.5 (texp2 = -7).
+ * The exchange then treats kappa_P implicitly, with the d kappa_P/dT term of eq 33, and evaluates
+ * kappa_F at the updated temperature. */
+void orc_set_opacity_law_T(orc_grid *g, double kP0, double kR0, double rho0, int exponent, double T0, int texp2)
+{
+    orc_set_opacity_law(g, kP0, kR0, rho0, exponent);
+    g->opac_T0 = T0; g->opac_texp2 = texp2;
+}
+
+/* floor of the HLL wavespeed in units of c_hat (reading R5: 0.1); exposed for the sensitivity pin only */
+void orc_set_wavespeed_floor(orc_grid *g, double s_floor) { g->s_floor = s_floor; }
+
+/* worker threads of the `omp parallel for` loops (results do not depend on it) */
+#ifdef _OPENMP
+#include <omp.h>
+void orc_set_threads(int n) { omp_set_num_threads(n < 1 ? 1 : n); }
+int  orc_get_threads(void) { return omp_get_max_threads(); }
+#else
+void orc_set_threads(int n) { (void)n; }
+int  orc_get_threads(void) { return 1; }
+#endif
 
 void orc_set_field(orc_grid *g, int field, const double *interior)
 {
@@ -137,6 +161,8 @@ static void fill_one(orc_grid *g, double *a, int comp)
      * rule of the face the index lies beyond; equivalent to filling x, then y, then z in sequence.  A ghost cell
      * beyond a FIXED face is left as the caller stored it. */
     const int n[3] = { g->nx, g->ny, g->nz };
+    const long long ntot = orc_ncells_total(g);
+#pragma omp parallel for collapse(3) schedule(static) if (ntot > ORC_OMP_MIN)
     for (int k = -ORC_NG; k < g->nz + ORC_NG; ++k)
         for (int j = -ORC_NG; j < g->ny + ORC_NG; ++j)
             for (int i = -ORC_NG; i < g->nx + ORC_NG; ++i) {
@@ -174,6 +200,8 @@ double orc_cfl_dt(orc_grid *g)
 {
     double smax = 0.0;
     long long bad = 0;
+    const long long ntot = orc_ncells_total(g);
+#pragma omp parallel for collapse(3) schedule(static) reduction(max : smax) reduction(+ : bad) if (ntot > ORC_OMP_MIN)
     for (int k = 0; k < g->nz; ++k)
         for (int j = 0; j < g->ny; ++j)
             for (int i = 0; i < g->nx; ++i) {

@@ -1,6 +1,9 @@
 /* hydro.c -- CPU ORACLE (test infrastructure): PPM-MOL hydro step of PAPER.md:120-172.
  * See qk_oracle.h for the role of this code.  Every formula below is written in the
- * evaluation order DESIGN.md section 3 fixes; no FMA contraction (-ffp-contract=off). */
+ * evaluation order DESIGN.md section 3 fixes; no FMA contraction (-ffp-contract=off).
+ * The `omp parallel for` lines only deal independent cells / faces out to threads (every loop body writes its own
+ * cell and reads arrays finished by an earlier loop): the arithmetic per cell, and so every result bit, is the
+ * same for any thread count (tests/test_oracle_hydro.py::test_thread_count_does_not_change_a_bit). */
 #include <math.h>
 #include <stdlib.h>
 #include <string.h>
@@ -152,6 +155,7 @@ static int hydro_divergence(const orc_grid *g, double *const U[5], double *div[5
     for (int d = 0; d < 3; ++d) chid[d] = (double *)malloc(ntot * sizeof(double));
 
     /* 1. primitives everywhere (ghosts included) */
+#pragma omp parallel for schedule(static) reduction(max : rc) if (ntot > ORC_OMP_MIN)
     for (long long c = 0; c < ntot; ++c) {
         double Uc[5] = { U[0][c], U[1][c], U[2][c], U[3][c], U[4][c] }, Wc[5];
         orc_cons_to_prim(g->gamma, Uc, Wc);
@@ -164,6 +168,7 @@ static int hydro_divergence(const orc_grid *g, double *const U[5], double *div[5
     for (int d = 0; d < 3; ++d) {
         long long s = strides[d];
         for (long long c = 0; c < ntot; ++c) chid[d][c] = 1.0;
+#pragma omp parallel for collapse(3) schedule(static) if (ntot > ORC_OMP_MIN)
         for (int k = -NG; k < nz + NG; ++k)
             for (int j = -NG; j < ny + NG; ++j)
                 for (int i = -NG; i < nx + NG; ++i) {
@@ -176,6 +181,7 @@ static int hydro_divergence(const orc_grid *g, double *const U[5], double *div[5
                 }
     }
     for (long long c = 0; c < ntot; ++c) chi[c] = 1.0;
+#pragma omp parallel for collapse(3) schedule(static) if (ntot > ORC_OMP_MIN)
     for (int k = -1; k <= nz; ++k)
         for (int j = -1; j <= ny; ++j)
             for (int i = -1; i <= nx; ++i) {
@@ -194,6 +200,7 @@ static int hydro_divergence(const orc_grid *g, double *const U[5], double *div[5
         int t1 = (d + 1) % 3, t2 = (d + 2) % 3;
         int lo[3] = { 0, 0, 0 }, hi[3] = { nx, ny, nz };
         lo[d] = -1; hi[d] = nn[d] + 1;
+#pragma omp parallel for collapse(3) schedule(static) if (ntot > ORC_OMP_MIN)
         for (int k = lo[2]; k < hi[2]; ++k)
             for (int j = lo[1]; j < hi[1]; ++j)
                 for (int i = lo[0]; i < hi[0]; ++i) {
@@ -207,6 +214,7 @@ static int hydro_divergence(const orc_grid *g, double *const U[5], double *div[5
                     }
                 }
         lo[d] = 0;                                   /* face at the low side of cells 0..n */
+#pragma omp parallel for collapse(3) schedule(static) if (ntot > ORC_OMP_MIN)
         for (int k = lo[2]; k < hi[2]; ++k)
             for (int j = lo[1]; j < hi[1]; ++j)
                 for (int i = lo[0]; i < hi[0]; ++i) {
@@ -219,6 +227,7 @@ static int hydro_divergence(const orc_grid *g, double *const U[5], double *div[5
                     flux[1 + t2][c] = F[3]; flux[4][c] = F[4];
                 }
         /* accumulate: after d=0 div=dFx; d=1 div=dFx+dFy; d=2 div=(dFx+dFy)+dFz */
+#pragma omp parallel for collapse(3) schedule(static) if (ntot > ORC_OMP_MIN)
         for (int k = 0; k < nz; ++k)
             for (int j = 0; j < ny; ++j)
                 for (int i = 0; i < nx; ++i) {
@@ -257,6 +266,7 @@ int orc_hydro_step(orc_grid *g, double dt)
         if (stage == 1) orc_fill_boundary(g, ORC_FILL_HYDRO);
         int r = hydro_divergence(g, U, div);
         if (r) rc = r;
+#pragma omp parallel for collapse(3) schedule(static) if (ntot > ORC_OMP_MIN)
         for (int k = 0; k < nz; ++k)
             for (int j = 0; j < ny; ++j)
                 for (int i = 0; i < nx; ++i) {

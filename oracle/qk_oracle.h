@@ -1,6 +1,6 @@
 /* qk_oracle.h -- CPU ORACLE (test infrastructure, NOT the product).
  *
- * Plain, slow, single-threaded fp64 C restatement of the per-timestep uniform-grid
+ * Plain, slow fp64 C restatement of the per-timestep uniform-grid
  * cell update of Wibking & Krumholz, "QUOKKA" (arXiv:2110.01792), written from
  * /root/reference/PAPER.md (cited below as PAPER.md:<line>) and from the readings
  * listed in DESIGN.md section 3.  It exists so that the CUDA path can be checked
@@ -35,6 +35,8 @@ extern "C" {
 
 #define ORC_NG 4          /* ghost zones per side (BASELINE.json config 1) */
 #define ORC_NFIELDS 12    /* rho mx my mz E Er Fx Fy Fz kappaP kappaR src  */
+#define ORC_OMP_MIN 4096  /* boxes (ghosts included) below this many cells stay on one thread: the `omp parallel for`
+                             lines deal independent cells out to threads and change no result */
 
 enum { ORC_RHO = 0, ORC_MX, ORC_MY, ORC_MZ, ORC_E, ORC_ER, ORC_FX, ORC_FY, ORC_FZ,
        ORC_KP, ORC_KR,
@@ -46,8 +48,10 @@ enum { ORC_BC_PERIODIC = 0, ORC_BC_OUTFLOW = 1,
 enum { ORC_FLAG_TAU_CORR = 1, ORC_FLAG_STATIC_MATTER = 2, ORC_FLAG_NEWTON_LITERAL = 4,
        ORC_FLAG_PLM = 8,          /* piecewise-linear reconstruction with the MC limiter */
        ORC_FLAG_EDDINGTON = 16,   /* Eddington approximation chi = 1/3 (P_r = E_r/3)  */
-       ORC_FLAG_MINERBO = 32 };   /* Minerbo (1978) closure in its usual polynomial form
-                                     chi = 1/3 + (2/15) f^2 (3 - f + 3 f^2); NOT printed in PAPER.md (V3) */
+       ORC_FLAG_MINERBO = 32,     /* Minerbo (1978) closure in its usual polynomial form
+                                     chi = 1/3 + (2/15) f^2 (3 - f + 3 f^2): approximate, NOT printed in PAPER.md (V3) */
+       ORC_FLAG_NO_DKAPPA_DT = 64 }; /* oracle only: drop the d kappa_P/dT term of eq 33 from the Jacobian (the pin that
+                                        shows the term speeds up Newton's iteration compares against this) */
 enum { ORC_EOS_IDEAL = 0, ORC_EOS_ALPHA_T3 = 1 };   /* eq 55, PAPER.md:424 (oracle only) */
 enum { ORC_FILL_HYDRO = 1, ORC_FILL_RAD = 2, ORC_FILL_ALL = 7 }; /* bit 4: opacities */
 
@@ -61,6 +65,8 @@ typedef struct orc_grid {
     int newton_maxit, nsub_max;
     unsigned flags;
     int opac_exp; double opac_kP0, opac_kR0, opac_rho0;   /* opacity law (orc_set_opacity_law), opac_rho0 = 0: fields */
+    int opac_texp2; double opac_T0;                       /* ... times (T/T0)^(opac_texp2/2) (orc_set_opacity_law_T)  */
+    double s_floor;                                       /* HLL wavespeed floor / c_hat (reading R5: 0.1)           */
     int eos; double alpha;          /* ORC_EOS_ALPHA_T3: E_g = alpha T^4 / 4           */
     double S_src;                   /* S of eq 27 for the cell orc_exchange_cell is called on; orc_exchange sets it
                                        to dt * f[ORC_SRC][cell] (0 in every BASELINE config)                  */
@@ -82,6 +88,10 @@ void   orc_set_constants(orc_grid *g, double a_rad, double kB_mu);
 void   orc_set_params(orc_grid *g, double cfl, double newton_tol, int newton_maxit, int nsub_max, unsigned flags);
 void   orc_set_eos(orc_grid *g, int eos, double alpha);
 void   orc_set_opacity_law(orc_grid *g, double kP0, double kR0, double rho0, int exponent);
+void   orc_set_opacity_law_T(orc_grid *g, double kP0, double kR0, double rho0, int exponent, double T0, int texp2);
+void   orc_set_wavespeed_floor(orc_grid *g, double s_floor);
+void   orc_set_threads(int n);
+int    orc_get_threads(void);
 int    orc_set_face_bc(orc_grid *g, const int bc6[6]);   /* 0 ok, 1 if periodic is not on both faces of an axis */
 void   orc_set_field(orc_grid *g, int field, const double *interior);
 void   orc_get_field(const orc_grid *g, int field, double *interior);
@@ -114,6 +124,11 @@ void   orc_closure_k(unsigned flags, const double fvec[3], int n, double T_col[3
 void   orc_rad_phys_flux(double c, double c_hat, const double S[4], int n, double G[4], double *Tnn);
 int    orc_rad_hll(double c, double c_hat, const double SL[4], const double SR[4], int n,
                    double tau_face, unsigned flags, double G[4]);
+int    orc_rad_hll_floor(double c, double c_hat, const double SL[4], const double SR[4], int n,
+                         double tau_face, unsigned flags, double s_floor, double G[4]);
+double orc_temp_power(double T, double T0, int n2);
+void   orc_opacity_density_part(const orc_grid *g, double rho, double *kP, double *kR);
+double orc_gas_temperature(const orc_grid *g, double rho, const double m[3], double E);
 int    orc_exchange_cell(const orc_grid *g, double dt, double rho, double m[3], double *E,
                          double *Er, double F[3], double kP, double kR, int *iters);
 

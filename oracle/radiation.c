@@ -94,19 +94,19 @@ void orc_rad_phys_flux(double c, double c_hat, const double S[4], int n, double 
     if (Tnn) *Tnn = T[n];
 }
 
-/* HLL flux with wavespeeds +-S, S = max(c_hat sqrt(Tnn_L), c_hat sqrt(Tnn_R), 0.1 c_hat),
+/* HLL flux with wavespeeds +-S, S = max(c_hat sqrt(Tnn_L), c_hat sqrt(Tnn_R), s_floor c_hat), s_floor = 0.1,
  * Eddington factors frozen.  With S_L = -S_R the HLL formula is
  * G = (G_L+G_R)/2 - (S/2)(U_R-U_L).  Optical-depth correction: the E_r
  * dissipation is scaled by eps = min(1, 1/tau_face); it is disabled for the face when
  * either HLL star state it implies violates E*>0, |F*|<=cE*.  Forms are DESIGN.md
  * readings R5/R6 (PARITY UNPINNED).  Returns 1 if the guard fired. */
-int orc_rad_hll(double c, double c_hat, const double SL[4], const double SR[4], int n,
-                double tau_face, unsigned flags, double G[4])
+int orc_rad_hll_floor(double c, double c_hat, const double SL[4], const double SR[4], int n,
+                      double tau_face, unsigned flags, double s_floor, double G[4])
 {
     double GL[4], GR[4], TL, TR;
     rad_phys_flux_k(flags, c, c_hat, SL, n, GL, &TL);
     rad_phys_flux_k(flags, c, c_hat, SR, n, GR, &TR);
-    double S = max2(max2(c_hat * sqrt(TL), c_hat * sqrt(TR)), 0.1 * c_hat);
+    double S = max2(max2(c_hat * sqrt(TL), c_hat * sqrt(TR)), s_floor * c_hat);
     double UL[4] = { SL[0], (c * SL[0]) * SL[1], (c * SL[0]) * SL[2], (c * SL[0]) * SL[3] };
     double UR[4] = { SR[0], (c * SR[0]) * SR[1], (c * SR[0]) * SR[2], (c * SR[0]) * SR[3] };
     double diss = 0.5 * S;
@@ -133,6 +133,13 @@ int orc_rad_hll(double c, double c_hat, const double SL[4], const double SR[4], 
     return 0;
 }
 
+/* the same with the floor of reading R5, 0.1 c_hat */
+int orc_rad_hll(double c, double c_hat, const double SL[4], const double SR[4], int n,
+                double tau_face, unsigned flags, double G[4])
+{
+    return orc_rad_hll_floor(c, c_hat, SL, SR, n, tau_face, flags, 0.1, G);
+}
+
 /* div[m][cell] = ((dGx + dGy) + dGz) for the ghost-filled radiation state R=(E_r,F_x,F_y,F_z) */
 static int rad_divergence(orc_grid *g, double *const R[4], double *div[4])
 {
@@ -151,6 +158,7 @@ static int rad_divergence(orc_grid *g, double *const R[4], double *div[4])
         flux[m] = (double *)malloc(ntot * sizeof(double));
     }
     /* reconstruct in E_r and the reduced flux f = F_r/(c E_r) */
+#pragma omp parallel for schedule(static) if (ntot > ORC_OMP_MIN)
     for (long long cidx = 0; cidx < ntot; ++cidx) {
         double E = R[0][cidx], cE = g->c * E;
         S[0][cidx] = E;
@@ -166,6 +174,8 @@ static int rad_divergence(orc_grid *g, double *const R[4], double *div[4])
         long long s = strides[d];
         int lo[3] = { 0, 0, 0 }, hi[3] = { nx, ny, nz };
         lo[d] = -1; hi[d] = nn[d] + 1;
+        long long nfall = 0, nguard = 0;
+#pragma omp parallel for collapse(3) schedule(static) reduction(+ : nfall) if (ntot > ORC_OMP_MIN)
         for (int k = lo[2]; k < hi[2]; ++k)
             for (int j = lo[1]; j < hi[1]; ++j)
                 for (int i = lo[0]; i < hi[0]; ++i) {
@@ -180,16 +190,17 @@ static int rad_divergence(orc_grid *g, double *const R[4], double *div[4])
                     double f2 = (lo4[1] * lo4[1] + lo4[2] * lo4[2]) + lo4[3] * lo4[3];
                     if (f2 > 1.0 || !(lo4[0] > 0.0)) {
                         for (int m = 0; m < 4; ++m) lo4[m] = S[m][c];
-                        g->fallback_states++;
+                        nfall++;
                     }
                     f2 = (hi4[1] * hi4[1] + hi4[2] * hi4[2]) + hi4[3] * hi4[3];
                     if (f2 > 1.0 || !(hi4[0] > 0.0)) {
                         for (int m = 0; m < 4; ++m) hi4[m] = S[m][c];
-                        g->fallback_states++;
+                        nfall++;
                     }
                     for (int m = 0; m < 4; ++m) { sl[m][c] = lo4[m]; sr[m][c] = hi4[m]; }
                 }
         lo[d] = 0;
+#pragma omp parallel for collapse(3) schedule(static) reduction(+ : nguard) if (ntot > ORC_OMP_MIN)
         for (int k = lo[2]; k < hi[2]; ++k)
             for (int j = lo[1]; j < hi[1]; ++j)
                 for (int i = lo[0]; i < hi[0]; ++i) {
@@ -198,9 +209,11 @@ static int rad_divergence(orc_grid *g, double *const R[4], double *div[4])
                     double SR[4] = { sl[0][c], sl[1][c], sl[2][c], sl[3][c] };
                     double tau = (0.5 * (kR[c - s] * rho[c - s] + kR[c] * rho[c])) * g->dx;
                     double G[4];
-                    g->guard_faces += orc_rad_hll(g->c, g->c_hat, SL, SR, d, tau, g->flags, G);
+                    nguard += orc_rad_hll_floor(g->c, g->c_hat, SL, SR, d, tau, g->flags, g->s_floor, G);
                     for (int m = 0; m < 4; ++m) flux[m][c] = G[m];
                 }
+        g->fallback_states += nfall; g->guard_faces += nguard;
+#pragma omp parallel for collapse(3) schedule(static) if (ntot > ORC_OMP_MIN)
         for (int k = 0; k < nz; ++k)
             for (int j = 0; j < ny; ++j)
                 for (int i = 0; i < nx; ++i) {
@@ -216,20 +229,23 @@ static int rad_divergence(orc_grid *g, double *const R[4], double *div[4])
     return rc;
 }
 
-/* kappa = kappa0 q^|e| with q = rho/rho0 (e > 0) or rho0/rho (e < 0), by repeated multiplication, for the
- * interior cells, from the density the hydro step left (opacities are static during a radiation subcycle) */
+/* kappa = kappa0 (rho/rho0)^e (T/T0)^(texp2/2) (orc_opacity_density_part, orc_temp_power) for the interior cells,
+ * from the density and gas temperature the hydro step / the last exchange left (opacities are static during the
+ * transport part of a radiation subcycle) */
 static void apply_opacity_law(orc_grid *g)
 {
     if (!(g->opac_rho0 > 0.0)) return;
-    const int n = g->opac_exp < 0 ? -g->opac_exp : g->opac_exp;
     for (int k = 0; k < g->nz; ++k)
         for (int j = 0; j < g->ny; ++j)
             for (int i = 0; i < g->nx; ++i) {
                 long long c = ((long long)(k + NG) * (g->ny + 2 * NG) + (j + NG)) * (g->nx + 2 * NG) + (i + NG);
-                double rho = g->f[ORC_RHO][c];
-                double q = g->opac_exp < 0 ? g->opac_rho0 / rho : rho / g->opac_rho0;
-                double kp = g->opac_kP0, kr = g->opac_kR0;
-                for (int m = 0; m < n; ++m) { kp = kp * q; kr = kr * q; }
+                double rho = g->f[ORC_RHO][c], kp, kr;
+                orc_opacity_density_part(g, rho, &kp, &kr);
+                if (g->opac_texp2 != 0) {
+                    double m[3] = { g->f[ORC_MX][c], g->f[ORC_MY][c], g->f[ORC_MZ][c] };
+                    double tp = orc_temp_power(orc_gas_temperature(g, rho, m, g->f[ORC_E][c]), g->opac_T0, g->opac_texp2);
+                    kp = kp * tp; kr = kr * tp;
+                }
                 g->f[ORC_KP][c] = kp; g->f[ORC_KR][c] = kr;
             }
 }
@@ -258,6 +274,7 @@ int orc_rad_transport(orc_grid *g, double dt)
         if (stage == 1) orc_fill_boundary(g, ORC_FILL_RAD);
         int r = rad_divergence(g, R, div);
         if (r) rc = r;
+#pragma omp parallel for collapse(3) schedule(static) if (ntot > ORC_OMP_MIN)
         for (int k = 0; k < nz; ++k)
             for (int j = 0; j < ny; ++j)
                 for (int i = 0; i < nx; ++i) {

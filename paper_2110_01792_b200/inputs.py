@@ -73,7 +73,7 @@ def config1(n=32, seed=1001, noise=1e-3):
     vz = noise * rng.standard_normal(shape)
     P = np.ones(shape)
     params = dict(nx=n, ny=n, nz=n, dx=1.0 / n, gamma=gamma, c_hat=0.0, c=0.0, bc=BC_PERIODIC,
-                  cfl=0.3, flags=FLAG_TAU_CORR, name="config1_hydro_wave")
+                  cfl=0.3, flags=0, name="config1_hydro_wave")
     return params, _fill_missing(_hydro_fields(rho, vx, vy, vz, P, gamma), shape)
 
 
@@ -90,12 +90,13 @@ def config2(n=256, seed=1002, mach=2.0, kmax=16, shape=None):
     scale = mach * np.sqrt(gamma) / rms
     P = np.ones(shape)
     params = dict(nx=shape[2], ny=shape[1], nz=shape[0], dx=1.0 / shape[2], gamma=gamma, c_hat=0.0, c=0.0,
-                  bc=BC_PERIODIC, cfl=0.3, flags=FLAG_TAU_CORR, name="config2_hydro_turbulence")
+                  bc=BC_PERIODIC, cfl=0.3, flags=0, name="config2_hydro_turbulence")
     return params, _fill_missing(_hydro_fields(rho, v[0] * scale, v[1] * scale, v[2] * scale, P, gamma), shape)
 
 
-def config3(n=128, seed=1003, shape=None):
-    """BASELINE.json configs[2]: radiation only, static matter, outflow, c=1, c_hat=0.1."""
+def config3(n=128, seed=1003, shape=None, tau_corr=False):
+    """BASELINE.json configs[2]: radiation only, static matter, outflow, c=1, c_hat=0.1.
+    tau_corr=True switches on the optical-depth correction of reading R6 (off by default: DESIGN.md section 3)."""
     shape = shape or (n, n, n)
     gamma = 5.0 / 3.0
     rng = _rng(seed)
@@ -114,11 +115,11 @@ def config3(n=128, seed=1003, shape=None):
               "Fz": f * c * Er * nvec[2] / norm, "kappaP": kappa, "kappaR": kappa.copy()}
     params = dict(nx=shape[2], ny=shape[1], nz=shape[0], dx=dx, gamma=gamma, c_hat=c_hat, c=c,
                   bc=BC_OUTFLOW, cfl=0.3, a_rad=1.0, kB_mu=1.0,
-                  flags=FLAG_TAU_CORR | FLAG_STATIC_MATTER, name="config3_radiation_static")
+                  flags=FLAG_STATIC_MATTER | (FLAG_TAU_CORR if tau_corr else 0), name="config3_radiation_static")
     return params, _fill_missing(fields, shape)
 
 
-def config4(n=256, seed=1004, kmax=16, shape=None, chat_ratio=0.01):
+def config4(n=256, seed=1004, kmax=16, shape=None, chat_ratio=0.01, tau_corr=False):
     """BASELINE.json configs[3]/[4]: coupled RHD, periodic, c/c_s ~ 100, c_hat/c = 0.01."""
     shape = shape or (n, n, n)
     gamma = 5.0 / 3.0
@@ -144,7 +145,7 @@ def config4(n=256, seed=1004, kmax=16, shape=None, chat_ratio=0.01):
     fields = {"rho": rho, "mx": rho * vx, "my": rho * vy, "mz": rho * vz, "E": E, "Er": Er,
               "kappaP": kappa, "kappaR": kappa.copy()}
     params = dict(nx=shape[2], ny=shape[1], nz=shape[0], dx=dx, gamma=gamma, c_hat=c_hat, c=c,
-                  bc=BC_PERIODIC, cfl=0.3, a_rad=a_rad, kB_mu=kB_mu, flags=FLAG_TAU_CORR,
+                  bc=BC_PERIODIC, cfl=0.3, a_rad=a_rad, kB_mu=kB_mu, flags=FLAG_TAU_CORR if tau_corr else 0,
                   name="config4_rhd")
     return params, _fill_missing(fields, shape)
 
@@ -164,7 +165,7 @@ def sedov(n=256):
     P = np.where(r2 < 0.01, 10.0, 0.1)
     z = _zeros(shape)
     params = dict(nx=n, ny=n, nz=n, dx=2.0 / n, gamma=gamma, c_hat=0.0, c=0.0, bc=BC_PERIODIC,
-                  cfl=0.25, flags=FLAG_TAU_CORR, name="sedov")
+                  cfl=0.25, flags=0, name="sedov")
     return params, _fill_missing(_hydro_fields(np.ones(shape), z, z.copy(), z.copy(), P, gamma), shape)
 
 
@@ -176,8 +177,8 @@ def ragged_hydro(shape=(19, 22, 37), seed=7, bc=BC_PERIODIC, mach=1.5):
     return p, f
 
 
-def ragged_rhd(shape=(18, 21, 35), seed=11, bc=BC_PERIODIC):
-    p, f = config4(seed=seed, kmax=3, shape=shape)
+def ragged_rhd(shape=(18, 21, 35), seed=11, bc=BC_PERIODIC, tau_corr=False):
+    p, f = config4(seed=seed, kmax=3, shape=shape, tau_corr=tau_corr)
     p["bc"] = bc
     p["name"] = "ragged_rhd"
     return p, f

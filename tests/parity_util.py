@@ -19,7 +19,7 @@ def make_oracle(params, fields):
                c_hat=params.get("c_hat", 0.0), c=params.get("c", 0.0), bc=params.get("bc", 0))
     if "a_rad" in params:
         g.set_constants(params["a_rad"], params["kB_mu"])
-    g.set_params(cfl=params.get("cfl", 0.3), flags=params.get("flags", 1))
+    g.set_params(cfl=params.get("cfl", 0.3), flags=params.get("flags", 0))
     g.set_all(fields)
     return g
 

@@ -197,3 +197,116 @@ def test_source_term_of_eq27():
         if kappa > 0.0:
             assert np.abs(g.get_state(4) - E0).max() > 1e-3      # the gas does take up part of the injected energy
         g.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# temperature-dependent opacities: kappa_P implicit with the d kappa_P / dT term of eq 33,
+# kappa_F at the updated temperature
+# ------------------------------------------------------------------------------------------------
+def test_temperature_power_is_the_plain_power():
+    L = O.lib()
+    for n2 in range(-8, 9):
+        for T, T0 in ((3.7, 1.3), (0.02, 5.0), (2.75e7, 1e6)):
+            assert abs(L.orc_temp_power(T, T0, n2) / (T / T0) ** (0.5 * n2) - 1.0) < 1e-14
+    assert L.orc_temp_power(7.0, 2.0, 0) == 1.0
+
+
+def _kT_grid(texp2, flags=0, c=50.0, ch=5.0, kP0=2.0, kR0=3.0, rho0=1.5, erho=1, T0=0.8):
+    g = _cell_grid(c, ch, flags=flags, tol=1e-13)
+    g.L.orc_set_opacity_law_T(g.h, kP0, kR0, rho0, erho, T0, texp2)
+    return g
+
+
+def test_kappa_of_T_backward_euler_by_bisection():
+    """With kappa_P = kappa0 (rho/rho0)^e (T/T0)^s the backward-Euler system eq 26-27 (S = 0) still conserves
+    E_g + (c/c_hat) E_r and reduces to one scalar equation in T^(t+1),
+        C_v (T - T_0) + (c/c_hat) dt rho kappa_P(T) c_hat (a_r T^4 - E_r(T)) = 0,  E_r(T) from conservation,
+    solved here by bisection to 1e-15.  Newton's result must agree for Kramers-like (s = -3.5), s = +1/2, s = 2, and
+    kappa_F must be taken at the updated temperature: F^(t+1) = F / (1 + rho kappa_R(T^(t+1)) c_hat dt)."""
+    c, ch, gamma = 50.0, 5.0, 5 / 3
+    kP0, kR0, rho0, T0 = 2.0, 3.0, 1.5, 0.8
+    for texp2 in (-7, 1, 4):
+        for (rho, Tg, Er, dt) in ((1.0, 2.0, 0.5, 0.01), (3.0, 0.5, 4.0, 0.003), (0.7, 1.0, 1.0 + 1e-3, 10.0)):
+            g = _kT_grid(texp2)
+            Cv = rho / (gamma - 1.0)
+            Eg0 = Cv * Tg
+            kden_P, kden_R = kP0 * (rho / rho0), kR0 * (rho / rho0)
+            rc, m1, E1, Er1, F1, it = _cell(g, dt, rho, [0, 0, 0], Eg0, Er, [0.3, 0.0, 0.0], kden_P, kden_R)
+            assert rc == 0
+            Eg1 = E1 - 0.5 * (m1 @ m1) / rho           # the damped flux pushed the gas (eq 41-42)
+            Etot = Eg0 + (c / ch) * Er
+
+            def resid(T):
+                kap = kden_P * (T / T0) ** (0.5 * texp2)
+                Er_T = (Etot - Cv * T) * (ch / c)
+                return Cv * (T - Tg) + (c / ch) * dt * rho * kap * ch * (T ** 4 - Er_T)
+
+            lo, hi = 1e-8, Etot / Cv
+            assert resid(lo) < 0 < resid(hi)
+            for _ in range(300):
+                mid = 0.5 * (lo + hi)
+                if resid(mid) > 0: hi = mid
+                else: lo = mid
+            Tnew = 0.5 * (lo + hi)
+            assert abs(Eg1 / (Cv * Tnew) - 1.0) < 1e-11, (texp2, rho, Eg1 / (Cv * Tnew) - 1.0)
+            assert abs((E1 + (c / ch) * Er1) / Etot - 1.0) < 1e-13
+            kR_new = kden_R * (Tnew / T0) ** (0.5 * texp2)
+            assert abs(F1[0] / (0.3 / (1 + rho * kR_new * ch * dt)) - 1.0) < 1e-10
+
+
+def test_dkappa_dT_term_of_eq33_speeds_up_newton():
+    """The Jacobian with the d kappa_P/dT term (eq 33) is the exact one: Newton then converges quadratically, while
+    the Jacobian without it (ORC_FLAG_NO_DKAPPA_DT) only converges linearly -- same fixed point, more iterations."""
+    rng = np.random.default_rng(8)
+    tot_full = tot_frozen = 0
+    for _ in range(200):
+        rho, Tg = np.exp(rng.normal(0, 0.5)), 10.0 ** rng.uniform(-0.3, 0.3)
+        Er = Tg ** 4 * 10.0 ** rng.uniform(-1, 1)
+        dt = 10.0 ** rng.uniform(-3, 0)
+        Cv = rho / (5 / 3 - 1.0)
+        res = []
+        for flags in (0, O.FLAG_NO_DKAPPA_DT):
+            g = _kT_grid(-7, flags=flags)
+            rc, _, Eg1, Er1, _, it = _cell(g, dt, rho, [0, 0, 0], Cv * Tg, Er, [0, 0, 0], 2.0 * rho / 1.5, 3.0 * rho / 1.5)
+            assert rc == 0
+            res.append((Eg1, it))
+        assert abs(res[0][0] / res[1][0] - 1.0) < 1e-9
+        tot_full += res[0][1]; tot_frozen += res[1][1]
+    assert tot_full < 0.8 * tot_frozen, (tot_full, tot_frozen)
+
+
+def test_kappa_law_without_T_exponent_is_the_density_law_bitwise():
+    """texp2 = 0 must reproduce orc_set_opacity_law bit for bit over whole RHD steps (no stray arithmetic)."""
+    from paper_2110_01792_b200 import inputs as I
+    outs = []
+    for use_T in (False, True):
+        p, f = I.ragged_rhd(shape=(6, 7, 9))
+        g = O.Grid(p["nx"], p["ny"], p["nz"], p["dx"], p["gamma"], c_hat=p["c_hat"], c=p["c"], bc=p["bc"])
+        g.set_constants(p["a_rad"], p["kB_mu"]); g.set_params(flags=p["flags"]); g.set_all(f)
+        if use_T: g.set_opacity_law_T(40.0, 60.0, 1.0, -1, 1.0, 0)
+        else: g.set_opacity_law(40.0, 60.0, 1.0, -1)
+        for _ in range(2):
+            assert g.rhd_step(g.cfl_dt()) == 0
+        outs.append([g.get_state(k) for k in range(11)])
+        g.close()
+    assert all(np.array_equal(a, b) for a, b in zip(*outs))
+
+
+def test_kappa_of_T_rhd_steps_conserve_and_track_temperature():
+    """Kramers-like kappa ~ rho T^-3.5 over coupled RHD steps: total energy and momentum conserved to round-off on a
+    periodic box, and the stored kappa_R field equals the law at the gas temperature the subcycle started from."""
+    from paper_2110_01792_b200 import inputs as I
+    p, f = I.ragged_rhd(shape=(6, 7, 9))
+    g = O.Grid(p["nx"], p["ny"], p["nz"], p["dx"], p["gamma"], c_hat=p["c_hat"], c=p["c"], bc=p["bc"])
+    g.set_constants(p["a_rad"], p["kB_mu"]); g.set_params(flags=p["flags"]); g.set_all(f)
+    g.set_opacity_law_T(30.0, 30.0, 1.0, 1, 1.0, -7)
+    coc = p["c"] / p["c_hat"]
+    tot0 = (g.get_state(4) + coc * g.get_state(5)).sum()
+    mom0 = (g.get_state(1) + g.get_state(6) / (p["c"] * p["c_hat"])).sum()
+    for _ in range(3):
+        assert g.rhd_step(g.cfl_dt()) == 0
+    tot1 = (g.get_state(4) + coc * g.get_state(5)).sum()
+    mom1 = (g.get_state(1) + g.get_state(6) / (p["c"] * p["c_hat"])).sum()
+    assert abs(tot1 / tot0 - 1) < 1e-13 and abs(mom1 - mom0) < 1e-12 * np.abs(g.get_state(1)).sum()
+    assert g.info()["newton_fail_cells"] == 0
+    g.close()

@@ -68,7 +68,6 @@ def test_sound_wave_printed_errors(row):
     assert abs(e / printed - 1.0) < 0.05, (N, e, printed)
 
 
-@pytest.mark.slow
 def test_sound_wave_printed_error_1024():
     e = _sound_wave_error(1024)
     assert abs(e / 1.7e-11 - 1.0) < 0.05, e
@@ -170,7 +169,6 @@ def test_sod_against_exact_solution():
     assert 1.6 < errs[0] / errs[1] < 2.6 and 1.6 < errs[1] / errs[2] < 2.6, errs
 
 
-@pytest.mark.slow
 def test_strong_shock_tube_error_scale():
     """PAPER.md:313-315: (rho,p) = (10,100)|(1,1), 1000 cells on [0,5], x0=2, t=0.4, CFL 0.1;
     relative rms-of-L1 error printed as 1.12e-3 (gamma not printed; 1.4 assumed: weak pin, ~1e-3)."""
@@ -369,3 +367,25 @@ def test_cfl_dt_eq21():
     g.set_state(4, np.full(shape, P / (G53 - 1) + 0.5 * rho * 1.0))
     dt = g.cfl_dt()
     assert abs(dt - 0.3 * 0.25 / (1.0 + np.sqrt(G53 * P / rho))) < 1e-15
+
+
+def test_thread_count_does_not_change_a_bit():
+    """oracle loops over cells are dealt out to threads (omp parallel for): per-cell arithmetic is untouched, so one
+    thread and all threads give identical bits and identical integer diagnostics (CPU baseline)."""
+    from paper_2110_01792_b200 import inputs as I
+    n0 = O.get_threads()
+    outs = []
+    try:
+        for nt in (1, max(2, n0)):
+            O.set_threads(nt)
+            p, f = I.ragged_rhd(shape=(14, 15, 17), tau_corr=True)
+            g = O.Grid(p["nx"], p["ny"], p["nz"], p["dx"], p["gamma"], c_hat=p["c_hat"], c=p["c"], bc=p["bc"])
+            g.set_constants(p["a_rad"], p["kB_mu"]); g.set_params(flags=p["flags"]); g.set_all(f)
+            assert g.L.orc_ncells_total(g.h) > 4096          # above ORC_OMP_MIN: the parallel regions are active
+            for _ in range(2):
+                assert g.rhd_step(g.cfl_dt()) == 0
+            outs.append(([g.get_state(k) for k in range(9)], g.info()))
+            g.close()
+    finally:
+        O.set_threads(n0)
+    assert all(np.array_equal(a, b) for a, b in zip(outs[0][0], outs[1][0])) and outs[0][1] == outs[1][1]
