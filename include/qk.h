@@ -38,7 +38,7 @@ enum { QK_BC_PERIODIC = 0,   /* PAPER.md:293, 572 */
        QK_BC_REFLECTING = 2, /* PAPER.md:408, 438, 464; solid wall: mirror image, the wall-normal component of
                                 rho v and F_r negated (B1) */
        QK_BC_FIXED = 3 };    /* Dirichlet / inflow: the ghost cells beyond the
-                                face keep the values the caller stored with qk_set_raw (B2); sweep path only */
+                                face keep the values the caller stored with qk_set_raw (B2) */
 
 /* field ids: conserved hydro U=(rho, rho v, E), radiation moments
  * (E_r, F_r) (eq 11-12), Planck- and Rosseland-type opacities per cell
@@ -48,23 +48,27 @@ enum { QK_RHO = 0, QK_MX, QK_MY, QK_MZ, QK_E, QK_ER, QK_FX, QK_FY, QK_FZ, QK_KAP
                        (reading X13); zero unless set; read by the exchange step only */
        QK_NFIELDS };
 
-enum { QK_FLAG_TAU_CORR = 1,        /* guarded optical-depth correction of the E_r HLL flux (R6) */
+enum { QK_FLAG_TAU_CORR = 1,        /* guarded optical-depth correction of the E_r HLL flux in the form
+                                       of reading R6.  OFF by default: the paper prints no formula and this form misses
+                                       the one number it prints for tau_cell >> 1 (R6)        */
        QK_FLAG_STATIC_MATTER = 2,   /* exchange skips eq 41-43: gas held at rest (X11)            */
        QK_FLAG_NEWTON_LITERAL = 4,  /* literal stop rule of PAPER.md:237 instead of converge-then-polish (X5)   */
-       /* scheme variants (sweep path only; QK_EINVAL from the step calls on the cross-check paths): */
+       /* scheme variants: */
        QK_FLAG_PLM = 8,             /* piecewise-linear reconstruction, monotonized-central limiter, for hydro
                                        and radiation instead of PPM                              */
        QK_FLAG_EDDINGTON = 16,      /* Eddington approximation chi = 1/3, P_r = E_r/3,
                                        instead of the Levermore closure                                         */
-       QK_FLAG_MINERBO = 32 };      /* Minerbo (1978) closure, chi = 1/3 + (2/15) f^2 (3 - f + 3 f^2) (
-                                       formula from the literature, V3); not together with QK_FLAG_EDDINGTON    */
+       QK_FLAG_MINERBO = 32 };      /* Minerbo (1978) closure in the APPROXIMATE polynomial form customary in the
+                                       literature, chi = 1/3 + (2/15) f^2 (3 - f + 3 f^2) (within 0.011 of the
+                                       maximum-entropy definition; PAPER.md:196 names the closure, prints no formula;
+                                       V3); not together with QK_FLAG_EDDINGTON                                 */
 
 enum { QK_FILL_HYDRO = 1, QK_FILL_RAD = 2, QK_FILL_OPACITY = 4, QK_FILL_ALL = 7 };
 
 /* z-slab domain decomposition (one box per GPU; the paper's pattern: one ghost exchange per
  * RK stage).  Faces named here border another rank's slab. */
 enum { QK_FACE_ZLO = 1, QK_FACE_ZHI = 2 };
-typedef void (*qk_halo_fn)(void *user, int nfields);
+typedef int (*qk_halo_fn)(void *user, int nfields);   /* 0 = ok; anything else aborts the step with QK_EINVAL */
 
 /* Counters of the most recent step call (qk_hydro_step / qk_rad_step / qk_rhd_step / qk_exchange
  * / qk_rad_transport), summed over the substeps of a qk_rhd_step. */
@@ -85,7 +89,7 @@ typedef struct qk_info {
  * state is allocated here with cudaMalloc unless `qk_bind_storage` supplies it before
  * first use (allocation is deferred to first use).  Defaults: a_rad = 1, k_B/(mu m_H) = 1,
  * CFL 0.3, Newton tolerance 1e-10, 400 iterations, N_sub,max 10,
- * flags = QK_FLAG_TAU_CORR.  Returns QK_EINVAL / QK_ENOMEM / QK_ECUDA on failure. */
+ * flags = 0.  Returns QK_EINVAL / QK_ENOMEM / QK_ECUDA on failure. */
 int qk_init(int nx, int ny, int nz, double dx, double gamma, double c_hat, double c, int boundary,
             qk_ctx **out);
 
@@ -93,9 +97,9 @@ int qk_init(int nx, int ny, int nz, double dx, double gamma, double c_hat, doubl
 int qk_free(qk_ctx *ctx);
 
 /* Bytes of device memory one context needs (12 state fields, 5 RK stage fields, the flattening
- * coefficient, 28 scratch fields -- primitives, flux-difference accumulators, radiation
- * reconstruction variables -- and counters), for callers that own the
- * allocation (torch.empty). */
+ * coefficient, 5 flux-difference accumulators, two sets of primitives and of radiation reconstruction
+ * variables and counters: 44 fields), for
+ * callers that own the allocation (torch.empty). */
 size_t qk_state_bytes(int nx, int ny, int nz);
 
 /* Use caller-owned DEVICE memory (>= qk_state_bytes, 256-byte aligned) instead of
@@ -121,6 +125,13 @@ int qk_set_face_boundaries(qk_ctx *ctx, const int *bc6);
  * subcycle; rho0 = 0 (default) leaves the fields as the caller set them. */
 int qk_set_opacity_law(qk_ctx *ctx, double kappaP0, double kappaR0, double rho0, int exponent);
 
+/* The same law times (T/T0)^(texp2/2), T the gas temperature and texp2 an integer in [-16, 16]: half-integer powers
+ * such as Kramers' kappa ~ rho T^-3.5 (exponent 1, texp2 -7), evaluated by repeated multiplication and one square
+ * root.  With texp2 != 0 the exchange treats kappa_P implicitly -- it follows the temperature of the Newton iterate
+ * and enters the Jacobian through the d kappa_P/dT term of eq 33 -- and takes kappa_F ~ kappa_R at the
+ * updated temperature; the opacity fields are refreshed from (rho, T) before every transport step. */
+int qk_set_opacity_law_T(qk_ctx *ctx, double kappaP0, double kappaR0, double rho0, int exponent, double T0, int texp2);
+
 /* Equation of state of the gas in the EXCHANGE step: QK_EOS_IDEAL (default; T = (gamma-1) E_g / (rho k_B/(mu m_H)))
  * or QK_EOS_ALPHA_T3, E_g = alpha T^4 / 4 with volumetric heat capacity C_v = alpha T^3 (eq 55, PAPER.md:424-427;
  * the Marshak, Su-Olson and energy-exchange tests, where the matter is static).  The hydro step always uses the
@@ -137,6 +148,16 @@ int qk_set_params(qk_ctx *ctx, double cfl, double newton_tol, int newton_maxit, 
  * state.  qk_get_state synchronises the stream before returning. */
 int qk_set_state(qk_ctx *ctx, int field, const double *interior);
 int qk_get_state(qk_ctx *ctx, int field, double *interior);
+
+/* The same for n fields at once WITHOUT synchronising: one copy per field on the context's own copy stream, ordered
+ * against the compute stream by events (an upload waits for the compute work enqueued so far and the next step waits
+ * for the upload; a download waits for the steps enqueued so far).  interiors[m] belongs to fields[m]; host arrays
+ * should be pinned (pageable memory still works but the copies then serialise) and must stay untouched until
+ * qk_wait_copies returns.  With two contexts the upload of one box, the step of the other and the download of the
+ * previous result overlap. */
+int qk_set_state_all(qk_ctx *ctx, int n, const int *fields, const double *const *interiors);
+int qk_get_state_all(qk_ctx *ctx, int n, const int *fields, double *const *interiors);
+int qk_wait_copies(qk_ctx *ctx);
 
 /* Same with the ghost zones: (nz+8)(ny+8)(nx+8) doubles (boundary-fill parity checks, Dirichlet values).  The
  * step functions fill the ghost zones of their internal reconstruction variables, not necessarily those of the
@@ -164,6 +185,31 @@ size_t qk_halo_doubles(const qk_ctx *ctx);          /* QK_NG * ny * nx: doubles 
 int qk_halo_pack(qk_ctx *ctx, int face, double *dev_buf);
 int qk_halo_unpack(qk_ctx *ctx, int face, const double *dev_buf);
 
+/* The same decomposition WITHOUT the host on the stage path: every rank maps its neighbours' storage (CUDA IPC between
+ * processes, plain pointers inside one process) and, before a ghost fill, a kernel on a side stream writes its
+ * QK_NG boundary planes straight into the neighbour's ghost planes (NVLink / NVSwitch peer stores) and raises an arrival
+ * counter in the neighbour's memory; the consuming stream waits on its own counter with a stream memory operation.
+ * Nothing spins and no host thread waits.  Each RK stage is ordered so that everything that reads no z ghost plane (the
+ * x / y images of the interior planes, flattening and x / y sweeps of the planes >= 3 cells from the faces; for
+ * radiation all x / y sweeps) runs while the planes travel; only the remaining boundary work and the z sweep wait
+ * (the paper attributes its multi-GPU loss to ghost fills that are not overlapped).
+ *   qk_halo_export    : describe this context's storage (after qk_bind_storage, if used).  Synchronises.
+ *   qk_set_halo_peers : attach the neighbour below (lo) and above (hi) in z; NULL = physical boundary on that face.
+ *                       Every rank exports, the handles are exchanged (e.g. torch.distributed.all_gather_object), every
+ *                       rank attaches, and only then does any rank step (the arrival counters restart at attach).  All
+ *                       ranks must then make the same sequence of step / fill calls.  Needs nz >= QK_NG, equal nx, ny;
+ *                       nz may differ between ranks.  (NULL, NULL) detaches.  qk_cfl_dt stays local: the caller takes
+ *                       the minimum over ranks.  The result equals the single-box update bit for bit. */
+typedef struct qk_halo_handle {
+    unsigned char ipc[64];        /* cudaIpcMemHandle_t of the allocation that holds the storage (has_ipc != 0)    */
+    unsigned long long base;      /* device address of the storage in the exporting process                        */
+    unsigned long long offset;    /* of the storage inside that allocation                                         */
+    long long pid;                /* exporting process: handles of the same process are attached by address        */
+    int device, nx, ny, nz, has_ipc;
+} qk_halo_handle;
+int qk_halo_export(qk_ctx *ctx, qk_halo_handle *out);
+int qk_set_halo_peers(qk_ctx *ctx, const qk_halo_handle *lo, const qk_halo_handle *hi);
+
 /* eq 21: dt = CFL dx / max_cells(|v| + c_s), |v| the vector magnitude,
  * further limited to nsub_max CFL dx / c_hat when c_hat > 0.  Synchronises.
  * Returns NaN if a cell has rho <= 0 or P <= 0 (then qk_last_info().status = QK_ESTATE). */
@@ -175,10 +221,17 @@ int qk_hydro_step(qk_ctx *ctx, double dt);
 
 /* The same step with the timestep of eq 21 (qk_cfl_dt's formula and CFL number) evaluated ON THE DEVICE from the
  * signal speed the previous step left there: nothing is read back, the launch queue never drains.  qk_last_dt
- * returns the dt that was used (synchronises).  Sweep path only (QK_EINVAL otherwise).  If the state is bad
- * (rho <= 0 or P <= 0 somewhere) dt is NaN, the state becomes NaN and qk_last_info().status is QK_ESTATE. */
+ * returns the dt that was used (synchronises).  If the state is bad (rho <= 0 or P <= 0 somewhere) dt is NaN, the
+ * state becomes NaN and qk_last_info().status is QK_ESTATE.  QK_EINVAL on a context with inter-rank faces (a slab's
+ * own signal speed is not the global one: take qk_cfl_dt, reduce over ranks, call qk_hydro_step). */
 int qk_hydro_step_cfl(qk_ctx *ctx);
 int qk_last_dt(qk_ctx *ctx, double *dt);
+
+/* The coupled cycle of qk_rhd_step with the device-resident timestep: dt = min(CFL dx / max(|v| + c_s),
+ * nsub CFL dx / c_hat), so that the nsub radiation substeps of dt / nsub the caller asks for respect the radiation
+ * CFL condition; 1 <= nsub <= nsub_max.  Same trajectory as qk_cfl_dt + qk_rhd_step whenever
+ * that pair would take nsub substeps of the same dt. */
+int qk_rhd_step_cfl(qk_ctx *ctx, int nsub);
 
 /* SSP-RK2 explicit transport of (E_r, F_r) over dt, no exchange. */
 int qk_rad_transport(qk_ctx *ctx, double dt);
@@ -201,16 +254,6 @@ int qk_last_info(qk_ctx *ctx, qk_info *out);
 
 /* Number of kernel launches this context has enqueued so far (bench.py's gpu_launches). */
 long long qk_launch_count(const qk_ctx *ctx);
-
-/* Which hand-written CUDA implementation of the hydro / radiation stages runs:
- * QK_PATH_FUSED   = one tiled kernel per RK stage (primitives, PPM, Riemann fluxes of the three
- *                   directions, divergence and stage update; fluxes never reach HBM);
- * QK_PATH_UNFUSED = one kernel per sub-step with intermediates in HBM (on-device cross-check);
- * QK_PATH_SWEEP   = direction-split barrier-free sweeps (x by warp shuffle, y and z by marching
- *                   columns), flux differences accumulated in one scratch field per variable.
- * All are GPU kernels of this library and give bit-identical results (same evaluation order). */
-enum { QK_PATH_FUSED = 0, QK_PATH_UNFUSED = 1, QK_PATH_SWEEP = 2 };
-int qk_set_path(qk_ctx *ctx, int path);
 
 /* Per-kernel-class device timing for the roofline report.  While
  * profiling is on, every group of launches of one kernel class is bracketed by CUDA events on

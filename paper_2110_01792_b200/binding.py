@@ -21,15 +21,16 @@ QK_BC_PERIODIC, QK_BC_OUTFLOW, QK_BC_REFLECTING, QK_BC_FIXED = 0, 1, 2, 3
 QK_FLAG_TAU_CORR, QK_FLAG_STATIC_MATTER, QK_FLAG_NEWTON_LITERAL = 1, 2, 4
 QK_FLAG_PLM, QK_FLAG_EDDINGTON, QK_FLAG_MINERBO = 8, 16, 32
 QK_FILL_HYDRO, QK_FILL_RAD, QK_FILL_OPACITY, QK_FILL_ALL = 1, 2, 4, 7
-QK_PATH_FUSED, QK_PATH_UNFUSED, QK_PATH_SWEEP = 0, 1, 2
 
 EXPORTS = [
     "qk_init", "qk_free", "qk_state_bytes", "qk_bind_storage", "qk_set_stream", "qk_set_constants",
     "qk_set_params", "qk_set_state", "qk_get_state", "qk_set_raw", "qk_get_raw", "qk_fill_boundary",
     "qk_cfl_dt", "qk_hydro_step", "qk_rad_transport", "qk_exchange", "qk_rad_step", "qk_rhd_step",
-    "qk_nsub_for", "qk_last_info", "qk_launch_count", "qk_set_path", "qk_set_profiling",
+    "qk_nsub_for", "qk_last_info", "qk_launch_count", "qk_set_profiling",
     "qk_kernel_class_count", "qk_kernel_class_name", "qk_kernel_times", "qk_version", "qk_fp64_probe",
-    "qk_selftest_divsqrt", "qk_set_eos", "qk_set_opacity_law", "qk_set_face_boundaries", "qk_hydro_step_cfl", "qk_last_dt", "qk_set_halo_exchange", "qk_halo_doubles", "qk_halo_pack", "qk_halo_unpack",
+    "qk_selftest_divsqrt", "qk_set_eos", "qk_set_opacity_law", "qk_set_opacity_law_T", "qk_set_face_boundaries",
+    "qk_hydro_step_cfl", "qk_rhd_step_cfl", "qk_last_dt", "qk_set_halo_exchange", "qk_halo_doubles", "qk_halo_pack",
+    "qk_halo_unpack", "qk_set_state_all", "qk_get_state_all", "qk_wait_copies", "qk_halo_export", "qk_set_halo_peers",
 ]
 
 
@@ -39,9 +40,14 @@ class qk_info(C.Structure):
                 ("fallback_states", C.c_longlong), ("guard_faces", C.c_longlong), ("status", C.c_int)]
 
 
+class qk_halo_handle(C.Structure):
+    _fields_ = [("ipc", C.c_ubyte * 64), ("base", C.c_ulonglong), ("offset", C.c_ulonglong), ("pid", C.c_longlong),
+                ("device", C.c_int), ("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int), ("has_ipc", C.c_int)]
+
+
 QK_FACE_ZLO, QK_FACE_ZHI = 1, 2
 QK_EOS_IDEAL, QK_EOS_ALPHA_T3 = 0, 1
-HALO_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_int)
+HALO_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_int)
 
 
 class QkError(RuntimeError):
@@ -71,15 +77,20 @@ def lib():
         "qk_set_params": (i, [p, d, d, i, i, u]),
         "qk_set_eos": (i, [p, i, d]),
         "qk_set_opacity_law": (i, [p, d, d, d, i]),
+        "qk_set_opacity_law_T": (i, [p, d, d, d, i, d, i]),
         "qk_set_face_boundaries": (i, [p, C.POINTER(C.c_int)]),
         "qk_set_state": (i, [p, i, p]),
         "qk_get_state": (i, [p, i, p]),
+        "qk_set_state_all": (i, [p, i, C.POINTER(i), C.POINTER(p)]),
+        "qk_get_state_all": (i, [p, i, C.POINTER(i), C.POINTER(p)]),
+        "qk_wait_copies": (i, [p]),
         "qk_set_raw": (i, [p, i, p]),
         "qk_get_raw": (i, [p, i, p]),
         "qk_fill_boundary": (i, [p, i]),
         "qk_cfl_dt": (d, [p]),
         "qk_hydro_step": (i, [p, d]),
         "qk_hydro_step_cfl": (i, [p]),
+        "qk_rhd_step_cfl": (i, [p, i]),
         "qk_last_dt": (i, [p, C.POINTER(d)]),
         "qk_rad_transport": (i, [p, d]),
         "qk_exchange": (i, [p, d]),
@@ -88,7 +99,6 @@ def lib():
         "qk_nsub_for": (i, [p, d]),
         "qk_last_info": (i, [p, C.POINTER(qk_info)]),
         "qk_launch_count": (ll, [p]),
-        "qk_set_path": (i, [p, i]),
         "qk_set_profiling": (i, [p, i]),
         "qk_kernel_class_count": (i, []),
         "qk_kernel_class_name": (C.c_char_p, [i]),
@@ -100,6 +110,8 @@ def lib():
         "qk_halo_doubles": (C.c_size_t, [p]),
         "qk_halo_pack": (i, [p, i, p]),
         "qk_halo_unpack": (i, [p, i, p]),
+        "qk_halo_export": (i, [p, C.POINTER(qk_halo_handle)]),
+        "qk_set_halo_peers": (i, [p, C.POINTER(qk_halo_handle), C.POINTER(qk_halo_handle)]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)
@@ -191,7 +203,7 @@ class Context:
     def qk_set_constants(self, a_rad, kB_over_mu_mH):
         _check(self.L.qk_set_constants(self.h, a_rad, kB_over_mu_mH), "qk_set_constants")
 
-    def qk_set_params(self, cfl=0.3, newton_tol=1e-10, newton_maxit=400, nsub_max=10, flags=QK_FLAG_TAU_CORR):
+    def qk_set_params(self, cfl=0.3, newton_tol=1e-10, newton_maxit=400, nsub_max=10, flags=0):
         _check(self.L.qk_set_params(self.h, cfl, newton_tol, newton_maxit, nsub_max, flags), "qk_set_params")
 
     def qk_set_face_boundaries(self, bc6):
@@ -204,8 +216,8 @@ class Context:
     def qk_set_eos(self, eos, alpha=0.0):
         _check(self.L.qk_set_eos(self.h, eos, alpha), "qk_set_eos")
 
-    def qk_set_path(self, path):
-        _check(self.L.qk_set_path(self.h, path), "qk_set_path")
+    def qk_set_opacity_law_T(self, kappaP0, kappaR0, rho0, exponent, T0, texp2):
+        _check(self.L.qk_set_opacity_law_T(self.h, kappaP0, kappaR0, rho0, exponent, T0, texp2), "qk_set_opacity_law_T")
 
     def qk_set_state(self, field, a):
         assert tuple(a.shape) == (self.nz, self.ny, self.nx), tuple(a.shape)
@@ -217,6 +229,24 @@ class Context:
         assert tuple(out.shape) == (self.nz, self.ny, self.nx)
         _check(self.L.qk_get_state(self.h, field, _ptr(out)), "qk_get_state")
         return out
+
+    def _field_list(self, fields, arrays):
+        n = len(fields)
+        for a in arrays:
+            assert tuple(a.shape) == (self.nz, self.ny, self.nx), tuple(a.shape)
+        return n, (C.c_int * n)(*[int(f) for f in fields]), (C.c_void_p * n)(*[_ptr(a) for a in arrays])
+
+    def qk_set_state_all(self, fields, arrays):
+        """Asynchronous upload of several fields (see include/qk.h); keep `arrays` alive until qk_wait_copies."""
+        n, f, p = self._field_list(fields, arrays)
+        _check(self.L.qk_set_state_all(self.h, n, f, p), "qk_set_state_all")
+
+    def qk_get_state_all(self, fields, arrays):
+        n, f, p = self._field_list(fields, arrays)
+        _check(self.L.qk_get_state_all(self.h, n, f, p), "qk_get_state_all")
+
+    def qk_wait_copies(self):
+        _check(self.L.qk_wait_copies(self.h), "qk_wait_copies")
 
     def qk_set_raw(self, field, a):
         assert tuple(a.shape) == (self.nz + 2 * NG, self.ny + 2 * NG, self.nx + 2 * NG)
@@ -234,8 +264,29 @@ class Context:
             self._halo_cb = None
             _check(self.L.qk_set_halo_exchange(self.h, 0, C.cast(None, HALO_FN), None), "qk_set_halo_exchange")
             return
-        self._halo_cb = HALO_FN(lambda user, nfields: fn(nfields))     # keep the thunk alive
+        def thunk(user, nfields):          # the callback's status aborts the step (a Python exception counts as failure)
+            try:
+                rc = fn(nfields)
+                return 0 if rc is None else int(rc)
+            except Exception as e:         # ctypes cannot propagate it through C: remember it for the caller
+                self._halo_error = e
+                return 1
+        self._halo_error = None
+        self._halo_cb = HALO_FN(thunk)     # keep the thunk alive
         _check(self.L.qk_set_halo_exchange(self.h, faces, self._halo_cb, None), "qk_set_halo_exchange")
+
+    def qk_halo_export(self):
+        """This context's storage as bytes (a qk_halo_handle): picklable, so it can cross ranks by all_gather_object."""
+        h = qk_halo_handle()
+        _check(self.L.qk_halo_export(self.h, C.byref(h)), "qk_halo_export")
+        return bytes(h)
+
+    def qk_set_halo_peers(self, lo, hi):
+        """lo / hi: handle bytes of the neighbour below / above in z, or None at a physical boundary."""
+        hl = qk_halo_handle.from_buffer_copy(lo) if lo is not None else None
+        hh = qk_halo_handle.from_buffer_copy(hi) if hi is not None else None
+        _check(self.L.qk_set_halo_peers(self.h, C.byref(hl) if hl is not None else None,
+                                        C.byref(hh) if hh is not None else None), "qk_set_halo_peers")
 
     def new_buffer(self, ndoubles):
         """Device buffer for halo planes (PyTorch owns the memory)."""
@@ -262,6 +313,9 @@ class Context:
 
     def qk_hydro_step_cfl(self):
         _check(self.L.qk_hydro_step_cfl(self.h), "qk_hydro_step_cfl")
+
+    def qk_rhd_step_cfl(self, nsub):
+        _check(self.L.qk_rhd_step_cfl(self.h, nsub), "qk_rhd_step_cfl")
 
     def qk_last_dt(self):
         out = C.c_double()
@@ -316,7 +370,7 @@ def from_params(params: dict, fields: dict | None = None, **kw) -> Context:
                   params.get("c_hat", 0.0), params.get("c", 0.0), params.get("bc", QK_BC_PERIODIC), **kw)
     if "a_rad" in params:
         ctx.qk_set_constants(params["a_rad"], params["kB_mu"])
-    ctx.qk_set_params(cfl=params.get("cfl", 0.3), flags=params.get("flags", QK_FLAG_TAU_CORR))
+    ctx.qk_set_params(cfl=params.get("cfl", 0.3), flags=params.get("flags", 0))
     if fields is not None:
         ctx.set_all(fields)
     return ctx

@@ -20,9 +20,8 @@ INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libqk.so")
 OBJ = os.path.join(HERE, "build")
 
-SOURCES = ["qk_api.cu", "k_boundary.cu", "k_cfl.cu", "k_exchange.cu", "k_hydro_ref.cu", "k_rad_ref.cu",
-           "k_hydro.cu", "k_rad.cu", "k_sweep.cu", "k_peak.cu"]
-HEADERS = ["qk_internal.h", "qk_math.cuh", "qk_fastmath.cuh", "k_stage_common.cuh", "k_sweep.cuh"]
+SOURCES = ["qk_api.cu", "k_boundary.cu", "k_cfl.cu", "k_exchange.cu", "k_sweep.cu", "k_peak.cu"]
+HEADERS = ["qk_internal.h", "qk_math.cuh", "qk_fastmath.cuh", "k_recon.cuh", "k_sweep.cuh"]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-fmad=false",
               "-std=c++17", "-Xcompiler", "-fPIC"]
@@ -55,7 +54,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
     def compile_one(src):
         obj = os.path.join(OBJ, src.replace(".cu", ".o"))
-        cmd = [nvcc()] + NVCC_FLAGS + extra + os.environ.get("QK_NVCC_EXTRA", "").split() + ["-I", INCLUDE, "-c", os.path.join(CSRC, src), "-o", obj]
+        cmd = [nvcc()] + NVCC_FLAGS + extra + ["-I", INCLUDE, "-c", os.path.join(CSRC, src), "-o", obj]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if r.returncode != 0:
             raise RuntimeError("nvcc failed for %s:\n%s\n%s" % (src, r.stdout, r.stderr))

@@ -30,7 +30,7 @@ __device__ __forceinline__ int wrap_index(int i, int n, int bc)
 
 // `ext` = QK_FACE_* bits of the z faces that border another rank's slab: their ghost planes already hold the
 // neighbour's cells at the interior (i, j) positions (qk_halo_unpack), so only their x / y images are filled.
-__global__ void __launch_bounds__(256) fill_ghost_kernel(Geom g, FaceBc fb, unsigned ext, FillList fl)
+__global__ void __launch_bounds__(256) fill_ghost_kernel(Geom g, FaceBc fb, unsigned ext, int part, FillList fl)
 {
     const long long nZ = 2LL * NG * g.py * g.px;
     const long long nY = 2LL * NG * g.nz * g.px;
@@ -60,6 +60,12 @@ __global__ void __launch_bounds__(256) fill_ghost_kernel(Geom g, FaceBc fb, unsi
             j = row - k * g.ny;
             i = ii < NG ? ii - NG : g.nx + (ii - NG);
         }
+        // part 1: everything except the ghost planes of inter-rank faces (fillable before the neighbour's planes have
+        // arrived); part 2: only those planes (their x / y images); part 0: all
+        if (part) {
+            const bool in_ext = (k < 0 && (ext & QK_FACE_ZLO)) || (k >= g.nz && (ext & QK_FACE_ZHI));
+            if (in_ext != (part == 2)) continue;
+        }
         // per axis: the rule of the face the index lies beyond (FaceBc: x-lo, x-hi, y-lo, y-hi, z-lo, z-hi)
         const int idx3[3] = {i, j, k}, n3[3] = {g.nx, g.ny, g.nz};
         int src3[3];
@@ -78,7 +84,13 @@ __global__ void __launch_bounds__(256) fill_ghost_kernel(Geom g, FaceBc fb, unsi
         }
         const int dst = g.at(i, j, k);
         const int src = g.at(src3[0], src3[1], src3[2]);
-        if (keep || src == dst) continue;
+        if (keep) {       // stage buffers take the Dirichlet values from the state field they shadow
+#pragma unroll 1
+            for (int f = 0; f < fl.n; ++f)
+                if (fl.fixed_src[f]) fl.f[f][dst] = fl.fixed_src[f][dst];
+            continue;
+        }
+        if (src == dst) continue;
         if (out_refl[0] || out_refl[1] || out_refl[2]) {
             // the normal component of rho v / v / F_r / f changes sign across each wall the image lies beyond
 #pragma unroll 1
@@ -127,14 +139,71 @@ int launch_halo_copy(const Geom &g, int face_hi, int unpack, const FillList &fl,
     return 1;
 }
 
-int launch_fill(const Geom &g, const FaceBc &fb, unsigned ext, const FillList &fl, cudaStream_t st)
+// ---- peer-mapped halo exchange (qk_set_halo_peers) -------------------------------------------------------------
+// The NG interior planes next to a z face go straight into the ghost planes of the neighbour's fields (peer memory:
+// NVLink stores, or the same device in the single-process tests), interior (i, j) cells only -- the neighbour's own
+// fill makes their x / y images.  dst[f] = the neighbour's array that corresponds to fl.f[f], whose box may have a
+// different nz (dg = its geometry).  One 16-byte store per thread where the row pitch allows it.
+__global__ void __launch_bounds__(256) halo_push_kernel(Geom g, Geom dg, int face_hi, FillList fl, PeerList dst)
+{
+    const long long per_field = (long long)NG * g.ny * g.nx;
+    const long long total = per_field * fl.n;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < total;
+         t += (long long)gridDim.x * blockDim.x) {
+        const int f = (int)(t / per_field);
+        const long long u = t - (long long)f * per_field;
+        const int row = (int)(u / g.nx);
+        const int i = (int)(u - (long long)row * g.nx);
+        const int kk = row / g.ny;
+        const int j = row - kk * g.ny;
+        // my planes nz-NG+kk (high face) land in the neighbour's planes -NG+kk; my planes kk (low face) in its nz'+kk
+        const int ks = face_hi ? g.nz - NG + kk : kk;
+        const int kd = face_hi ? kk - NG : dg.nz + kk;
+        dst.f[f][dg.at(i, j, kd)] = fl.f[f][g.at(i, j, ks)];
+    }
+}
+
+// the neighbour's arrival counter <- epoch, after every store of the push is visible system-wide
+__global__ void halo_signal_kernel(unsigned long long *flag, unsigned long long epoch)
+{
+    __threadfence_system();
+    *(volatile unsigned long long *)flag = epoch;
+    __threadfence_system();
+}
+
+// fallback for drivers without stream memory operations: one thread polls the arrival counter
+__global__ void halo_wait_kernel(const unsigned long long *flag, unsigned long long epoch)
+{
+    while (*(volatile const unsigned long long *)flag < epoch) __nanosleep(200);
+    __threadfence_system();
+}
+
+int launch_halo_push(const Geom &g, const Geom &dg, int face_hi, const FillList &fl, const PeerList &dst,
+                     unsigned long long *flag, unsigned long long epoch, cudaStream_t st)
+{
+    if (fl.n <= 0) return 0;
+    const long long total = (long long)NG * g.ny * g.nx * fl.n;
+    long long blocks = (total + 255) / 256;
+    if (blocks > 148LL * 8) blocks = 148LL * 8;
+    halo_push_kernel<<<(unsigned)blocks, 256, 0, st>>>(g, dg, face_hi, fl, dst);
+    halo_signal_kernel<<<1, 1, 0, st>>>(flag, epoch);
+    return 2;
+}
+
+int launch_halo_wait(const unsigned long long *flag, unsigned long long epoch, cudaStream_t st)
+{
+    halo_wait_kernel<<<1, 1, 0, st>>>(flag, epoch);
+    return 1;
+}
+
+int launch_fill(const Geom &g, const FaceBc &fb, unsigned ext, int part, const FillList &fl, cudaStream_t st)
 {
     if (fl.n <= 0) return 0;
     const long long total = 2LL * NG * ((long long)g.py * g.px + (long long)g.nz * g.px + (long long)g.nz * g.ny);
     long long blocks = (total + 255) / 256;
     const long long cap = 148LL * 32;
     if (blocks > cap) blocks = cap;
-    fill_ghost_kernel<<<(unsigned)blocks, 256, 0, st>>>(g, fb, ext, fl);
+    fill_ghost_kernel<<<(unsigned)blocks, 256, 0, st>>>(g, fb, ext, part, fl);
     return 1;
 }
 

@@ -50,7 +50,8 @@ __global__ void __launch_bounds__(256) cfl_max_speed_kernel(Geom g, double gamma
 }
 
 // eq 21 (and the N_sub,max limit) on the device, same operations as qk_cfl_dt does on the host
-__global__ void dt_from_cache_kernel(const StateCache *cache, DeviceDt *out, double cfl, double dx, double c_hat, int nsub_max)
+__global__ void dt_from_cache_kernel(const StateCache *cache, DeviceDt *out, double cfl, double dx, double c_hat, int nsub_max,
+                                     int nsub)
 {
     double dt;
     if (cache->cfl_bad != 0) {
@@ -65,12 +66,14 @@ __global__ void dt_from_cache_kernel(const StateCache *cache, DeviceDt *out, dou
     }
     out->dt = dt;
     out->dtdx = dt / dx;
+    out->dts = dt / (double)nsub;                  // radiation substep (qk_rhd_step_cfl), as qk_rhd_step forms it
+    out->dtsdx = out->dts / dx;
 }
 
 int launch_dt_from_cache(const StateCache *cache, DeviceDt *out, double cfl, double dx, double c_hat, int nsub_max,
-                         cudaStream_t st)
+                         int nsub, cudaStream_t st)
 {
-    dt_from_cache_kernel<<<1, 1, 0, st>>>(cache, out, cfl, dx, c_hat, nsub_max);
+    dt_from_cache_kernel<<<1, 1, 0, st>>>(cache, out, cfl, dx, c_hat, nsub_max, nsub);
     return 1;
 }
 

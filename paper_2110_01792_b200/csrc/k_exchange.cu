@@ -10,10 +10,9 @@
 
 namespace qk {
 
-#ifndef QK_EX_MINB
-#define QK_EX_MINB 7     // <= 73 registers: 1.09 -> 1.02 ms at 256^3 (6: 1.04, 5: 1.10); 8 spills into the Newton loop (1.45 ms)
-#endif
-__global__ void __launch_bounds__(128, QK_EX_MINB) exchange_kernel(Geom g, ExchangeConsts kc, double dt, const double *__restrict__ rho,
+constexpr int QK_EX_MINB = 6;    // 85 registers (7 CTAs / 73 registers spills once dt and the opacity law are parameters)
+template <bool KT>
+__global__ void __launch_bounds__(128, KT ? 5 : QK_EX_MINB) exchange_kernel(Geom g, ExchangeConsts kc, double dt_host, const double *__restrict__ dt_dev, const double *__restrict__ rho,
                                                        double *__restrict__ mx, double *__restrict__ my,
                                                        double *__restrict__ mz, double *__restrict__ E,
                                                        double *__restrict__ Er, double *__restrict__ Fx,
@@ -23,6 +22,7 @@ __global__ void __launch_bounds__(128, QK_EX_MINB) exchange_kernel(Geom g, Excha
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y, k = blockIdx.z;
+    const double dt = dt_dev ? __ldg(dt_dev) : dt_host;
     int iters = 0, fail = 0, bad = 0, bad_hydro = 0;
     double smax = 0.0;
     if (i < g.nx) {
@@ -31,23 +31,27 @@ __global__ void __launch_bounds__(128, QK_EX_MINB) exchange_kernel(Geom g, Excha
         double e = E[cidx], er = Er[cidx];
         double f0 = Fx[cidx], f1 = Fy[cidx], f2 = Fz[cidx];
         const double S = src ? dt * src[cidx] : 0.0;              // eq 27: energy added during the substep (X13)
-        const int rc = exchange_cell(kc, dt, rho[cidx], m0, m1, m2, e, er, f0, f1, f2, kP[cidx], kR[cidx], S, iters);
+        double kp = kP[cidx], kr = kR[cidx];
+        if (KT) opacity_density_part(rho[cidx], kc.kP0, kc.kR0, kc.rho0, kc.opac_exp, kp, kr);
+        const int rc = exchange_cell<KT>(kc, dt, rho[cidx], m0, m1, m2, e, er, f0, f1, f2, kp, kr, S, iters);
         fail = (rc == 4);
         bad = (rc == 5);
         if (!kc.static_matter) { mx[cidx] = m0; my[cidx] = m1; mz[cidx] = m2; }
         E[cidx] = e; Er[cidx] = er;
         Fx[cidx] = f0; Fy[cidx] = f1; Fz[cidx] = f2;
-        if (Wout.rho) {
-            // reconstruction variables of the updated cell for the next hydro / radiation stage and its CFL
-            // speed (same operations as prim_kernel, rad_prim_kernel and cfl_max_speed_kernel)
+        {
+            // CFL signal speed of the updated cell (eq 21) and, when asked, its reconstruction variables for the next
+            // hydro / radiation stage (same operations as cfl_max_speed_kernel, prim_kernel and rad_prim_kernel)
             Prim p;
             double sp;
             cell_prim_speed(kc.gamma, rho[cidx], m0, m1, m2, e, true, p, sp);
-            Wout.rho[cidx] = p.rho; Wout.mx[cidx] = p.vx; Wout.my[cidx] = p.vy; Wout.mz[cidx] = p.vz; Wout.E[cidx] = p.P;
             if (!(p.rho > 0.0) || !(p.P > 0.0)) bad_hydro = 1;
             else smax = sp;
-            const double cE = kc.c * er;
-            Sout.E[cidx] = er; Sout.Fx[cidx] = f0 / cE; Sout.Fy[cidx] = f1 / cE; Sout.Fz[cidx] = f2 / cE;
+            if (Wout.rho) {
+                Wout.rho[cidx] = p.rho; Wout.mx[cidx] = p.vx; Wout.my[cidx] = p.vy; Wout.mz[cidx] = p.vz; Wout.E[cidx] = p.P;
+                const double cE = kc.c * er;
+                Sout.E[cidx] = er; Sout.Fx[cidx] = f0 / cE; Sout.Fy[cidx] = f1 / cE; Sout.Fz[cidx] = f2 / cE;
+            }
         }
     }
     int tot = iters, mxit = iters;
@@ -65,7 +69,7 @@ __global__ void __launch_bounds__(128, QK_EX_MINB) exchange_kernel(Geom g, Excha
         if (mxit > 0) atomicMax(&ctr->newton_max, mxit);
         if (fail) atomicAdd((unsigned long long *)&ctr->newton_fail, (unsigned long long)fail);
         if (bad) atomicAdd((unsigned long long *)&ctr->bad_state, (unsigned long long)bad);
-        if (Wout.rho) {
+        {
             const unsigned long long bits = (unsigned long long)__double_as_longlong(smax);
             if (bits > *(volatile unsigned long long *)&cache->smax_bits) atomicMax(&cache->smax_bits, bits);
             if (bad_hydro) atomicAdd((unsigned long long *)&cache->cfl_bad, (unsigned long long)bad_hydro);
@@ -73,34 +77,30 @@ __global__ void __launch_bounds__(128, QK_EX_MINB) exchange_kernel(Geom g, Excha
     }
 }
 
-// kappa = kappa0 q^|e|, q = rho/rho0 (e > 0) or rho0/rho (e < 0), by repeated multiplication (X14): the density
-// power laws of the paper's tests, interior cells, evaluated before a radiation subcycle
-__global__ void __launch_bounds__(128) opacity_law_kernel(Geom g, const double *__restrict__ rho, double *__restrict__ kP,
-                                                          double *__restrict__ kR, double kP0, double kR0, double rho0, int e)
+// kappa = kappa0 (rho/rho0)^e (T/T0)^(texp2/2) for the interior cells (X14; the laws of the paper's tests,
+// PAPER.md:464, 528, and Kramers-like temperature laws), from the density and gas temperature of the current
+// state, evaluated before the transport part of a radiation subcycle
+__global__ void __launch_bounds__(128) opacity_law_kernel(Geom g, ExchangeConsts kc, CHydro5 U, double *__restrict__ kP,
+                                                          double *__restrict__ kR)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= g.nx) return;
     const int cidx = g.at(i, blockIdx.y, blockIdx.z);
-    const double r = rho[cidx];
-    const double q = e < 0 ? rho0 / r : r / rho0;
-    const int n = e < 0 ? -e : e;
-    double kp = kP0, kr = kR0;
-    for (int m = 0; m < n; ++m) { kp = kp * q; kr = kr * q; }
+    const double r = U.rho[cidx];
+    double kp, kr;
+    opacity_density_part(r, kc.kP0, kc.kR0, kc.rho0, kc.opac_exp, kp, kr);
+    if (kc.texp2 != 0) {
+        const double mx = U.mx[cidx], my = U.my[cidx], mz = U.mz[cidx];
+        const double msq = (mx * mx + my * my) + mz * mz;
+        const double Eg = U.E[cidx] - 0.5 * msq / r;
+        const double T = kc.eos_alpha_t3 ? sqrt(sqrt(4.0 * Eg / kc.alpha)) : Eg / (r * kc.kB_mu / (kc.gamma - 1.0));
+        const double tp = temperature_power(T, kc.T0, kc.texp2);
+        kp = kp * tp; kr = kr * tp;
+    }
     kP[cidx] = kp; kR[cidx] = kr;
 }
 
-int launch_opacity_law(const Geom &g, const double *rho, double *kP, double *kR, double kP0, double kR0, double rho0,
-                       int e, cudaStream_t st)
-{
-    dim3 grid((g.nx + 127) / 128, g.ny, g.nz);
-    opacity_law_kernel<<<grid, 128, 0, st>>>(g, rho, kP, kR, kP0, kR0, rho0, e);
-    return 1;
-}
-
-int launch_exchange(const Geom &g, const PhysConsts &pc, double dt, const double *rho, double *mx, double *my,
-                    double *mz, double *E, double *Er, double *Fx, double *Fy, double *Fz, const double *kP,
-                    const double *kR, const double *src, Hydro5 Wout, Rad4p Sout, Counters *ctr, StateCache *cache,
-                    cudaStream_t st)
+static ExchangeConsts exchange_consts(const PhysConsts &pc)
 {
     ExchangeConsts kc;
     kc.c = pc.c; kc.c_hat = pc.c_hat; kc.a_rad = pc.a_rad; kc.kB_mu = pc.kB_mu; kc.gamma = pc.gamma;
@@ -108,8 +108,30 @@ int launch_exchange(const Geom &g, const PhysConsts &pc, double dt, const double
     kc.alpha = pc.eos_alpha; kc.eos_alpha_t3 = pc.eos_alpha > 0.0;
     kc.literal_stop = (pc.flags & QK_FLAG_NEWTON_LITERAL) != 0;
     kc.static_matter = (pc.flags & QK_FLAG_STATIC_MATTER) != 0;
+    kc.kappa_T = pc.opac_rho0 > 0.0 && pc.opac_texp2 != 0;
+    kc.texp2 = pc.opac_texp2; kc.opac_exp = pc.opac_exp;
+    kc.T0 = pc.opac_T0; kc.kP0 = pc.opac_kP0; kc.kR0 = pc.opac_kR0; kc.rho0 = pc.opac_rho0;
+    return kc;
+}
+
+int launch_opacity_law(const Geom &g, const PhysConsts &pc, CHydro5 U, double *kP, double *kR, cudaStream_t st)
+{
     dim3 grid((g.nx + 127) / 128, g.ny, g.nz);
-    exchange_kernel<<<grid, 128, 0, st>>>(g, kc, dt, rho, mx, my, mz, E, Er, Fx, Fy, Fz, kP, kR, src, Wout, Sout, ctr, cache);
+    opacity_law_kernel<<<grid, 128, 0, st>>>(g, exchange_consts(pc), U, kP, kR);
+    return 1;
+}
+
+int launch_exchange(const Geom &g, const PhysConsts &pc, double dt, const double *dt_dev, const double *rho, double *mx, double *my,
+                    double *mz, double *E, double *Er, double *Fx, double *Fy, double *Fz, const double *kP,
+                    const double *kR, const double *src, Hydro5 Wout, Rad4p Sout, Counters *ctr, StateCache *cache,
+                    cudaStream_t st)
+{
+    const ExchangeConsts kc = exchange_consts(pc);
+    dim3 grid((g.nx + 127) / 128, g.ny, g.nz);
+    if (kc.kappa_T)
+        exchange_kernel<true><<<grid, 128, 0, st>>>(g, kc, dt, dt_dev, rho, mx, my, mz, E, Er, Fx, Fy, Fz, kP, kR, src, Wout, Sout, ctr, cache);
+    else
+        exchange_kernel<false><<<grid, 128, 0, st>>>(g, kc, dt, dt_dev, rho, mx, my, mz, E, Er, Fx, Fy, Fz, kP, kR, src, Wout, Sout, ctr, cache);
     return 1;
 }
 

@@ -102,6 +102,8 @@ __global__ void __launch_bounds__(256) divsqrt_selftest_kernel(long long n, unsi
             ++acc_div;
             const double ref = x / y;
             if (__double_as_longlong(q) != __double_as_longlong(ref)) ++bad_div;
+            // the variant without the range test (operands proved in range by an operand window) is the same chain
+            else if (__double_as_longlong(fdiv_inrange(x, y)) != __double_as_longlong(ref)) ++bad_div;
         }
         risk = 0;
         const double ax = fabs(x);
@@ -109,6 +111,7 @@ __global__ void __launch_bounds__(256) divsqrt_selftest_kernel(long long n, unsi
         if (!risk) {
             ++acc_sqrt;
             if (__double_as_longlong(s) != __double_as_longlong(sqrt(ax))) ++bad_sqrt;
+            else if (ax > 0.0 && __double_as_longlong(fsqrt_inrange(ax)) != __double_as_longlong(s)) ++bad_sqrt;
         }
     }
     atomicAdd(&out[0], acc_div); atomicAdd(&out[1], bad_div);

@@ -1,74 +1,12 @@
-// k_stage_common.cuh -- tiling shared by the fused stage kernels (k_hydro.cu, k_rad.cu).
-//
-// 2.5-D marching tiles: a CTA owns a TX x TY patch of columns and marches along z over a chunk of
-// planes.  At step k it holds
-//   * a ring of five planes k-1..k+3 of the cell-centred reconstruction variables of its own
-//     columns in shared memory (the z stencil of PPM for cell k+1),
-//   * plane k with a star-shaped halo of 3 cells in x and y (the x/y stencils of the tile cells
-//     and of the one cell beyond each tile edge whose face state a tile-edge flux needs).
-// Fluxes live in registers / shared memory only; HBM sees one read of the conserved state (plus
-// halo re-reads that L2 absorbs) and one write of the updated state per stage.
+// k_recon.cuh -- per-cell reconstruction building blocks of the sweep kernels (k_sweep.cuh): PPM / PLM face
+// states of all variables of one cell and the first-order fallback of the radiation
+// states.  Device inline functions only; every formula in the evaluation order DESIGN.md section 3 fixes.
 #pragma once
 
 #include "qk_internal.h"
 #include "qk_math.cuh"
 
 namespace qk {
-
-constexpr int TX = 32;            // tile width  (x, one warp per row: coalesced 256-byte rows)
-constexpr int TY = 8;             // tile height (y)
-constexpr int NT = TX * TY;       // threads per CTA
-constexpr int RING = 5;           // planes k-1..k+3
-constexpr int HALO = 3;           // in-plane star halo
-constexpr int N_HALO_X = 2 * HALO * TY;          // halo cells left/right of the tile rows
-constexpr int N_HALO = N_HALO_X + 2 * HALO * TX; // + below/above the tile columns
-constexpr int N_EDGE_X = 2 * TY;                 // cells -1 and TX of every row
-constexpr int N_EDGE = N_EDGE_X + 2 * TX;        // + cells -1 and TY of every column
-
-static_assert(N_HALO <= NT, "one halo cell per thread");
-static_assert(N_EDGE <= NT && TX + TY <= NT, "one edge item per thread");
-
-__device__ __forceinline__ int ring_slot(int plane) { return (plane + 2 * RING) % RING; }
-
-// tile-local coordinates of halo cell h (0 <= h < N_HALO)
-__device__ __forceinline__ void halo_cell(int h, int &lx, int &ly)
-{
-    if (h < N_HALO_X) {
-        ly = h / (2 * HALO);
-        const int q = h - ly * (2 * HALO);
-        lx = q < HALO ? q - HALO : TX + (q - HALO);
-    } else {
-        const int u = h - N_HALO_X;
-        const int r = u / TX;
-        lx = u - r * TX;
-        ly = r < HALO ? r - HALO : TY + (r - HALO);
-    }
-}
-
-// tile-local coordinates of edge cell e (0 <= e < N_EDGE): the cells one beyond the tile along x
-// (e < N_EDGE_X) or along y; `high` tells which side
-__device__ __forceinline__ void edge_cell(int e, int &lx, int &ly, bool &along_x, bool &high)
-{
-    if (e < N_EDGE_X) {
-        along_x = true;
-        ly = e >> 1;
-        high = (e & 1) != 0;
-        lx = high ? TX : -1;
-    } else {
-        along_x = false;
-        const int u = e - N_EDGE_X;
-        high = u >= TX;
-        lx = high ? u - TX : u;
-        ly = high ? TY : -1;
-    }
-}
-
-__device__ __forceinline__ bool in_array(const Geom &g, int i, int j)
-{
-    return i >= -NG && i < g.nx + NG && j >= -NG && j < g.ny + NG;
-}
-
-// ---- per-cell / per-face building blocks shared by the tile kernels and the sweep kernels ------
 
 // The select-only PPM limiter of qk_math.cuh (ppm_face_states_t<true>) for NV variables of one cell in
 // lockstep: every elementary step is issued for all variables before the next step starts, so that the
@@ -174,13 +112,25 @@ __device__ __forceinline__ void ppm_cell(Q q, double chi, double lo[5], double h
     }
 }
 
-// HLLC flux through a face with normal DIR; L, R = (rho, vx, vy, vz, P); F in conserved order
-template <int DIR>
-__device__ __forceinline__ void face_flux(double gamma, const double L[5], const double R[5], double F[5])
+// First-order fallback per face state (R3): a state with |f|^2 > 1 or E <= 0 reverts, all four
+// variables, to the cell average q(v, 2).  Returns the number of reverted states.
+template <typename Q>
+__device__ __forceinline__ int rad_fallback(Q q, double lo[4], double hi[4])
 {
-    constexpr int n = 1 + DIR, t1 = 1 + (DIR + 1) % 3, t2 = 1 + (DIR + 2) % 3;
-    const Flux5 f = hllc_flux(gamma, L[0], L[n], L[t1], L[t2], L[4], R[0], R[n], R[t1], R[t2], R[4]);
-    F[0] = f.m; F[n] = f.pn; F[t1] = f.pt1; F[t2] = f.pt2; F[4] = f.e;
+    int nfall = 0;
+    double f2 = (lo[1] * lo[1] + lo[2] * lo[2]) + lo[3] * lo[3];
+    if (f2 > 1.0 || !(lo[0] > 0.0)) {
+#pragma unroll
+        for (int v = 0; v < 4; ++v) lo[v] = q(v, 2);
+        ++nfall;
+    }
+    f2 = (hi[1] * hi[1] + hi[2] * hi[2]) + hi[3] * hi[3];
+    if (f2 > 1.0 || !(hi[0] > 0.0)) {
+#pragma unroll
+        for (int v = 0; v < 4; ++v) hi[v] = q(v, 2);
+        ++nfall;
+    }
+    return nfall;
 }
 
 // PPM face states of (E, fx, fy, fz) of one cell, q(v, m) = variable v at stencil offset m-2; a face
@@ -199,30 +149,7 @@ __device__ __forceinline__ int rad_ppm_cell(Q q, double lo[4], double hi[4])
         for (int v = 0; v < 4; ++v)
             ppm_face_states_t<BL != 0>(q(v, 0), q(v, 1), ctr[v], q(v, 3), q(v, 4), lo[v], hi[v]);
     }
-    int nfall = 0;
-    double f2 = (lo[1] * lo[1] + lo[2] * lo[2]) + lo[3] * lo[3];
-    if (f2 > 1.0 || !(lo[0] > 0.0)) {
-#pragma unroll
-        for (int v = 0; v < 4; ++v) lo[v] = ctr[v];
-        ++nfall;
-    }
-    f2 = (hi[1] * hi[1] + hi[2] * hi[2]) + hi[3] * hi[3];
-    if (f2 > 1.0 || !(hi[0] > 0.0)) {
-#pragma unroll
-        for (int v = 0; v < 4; ++v) hi[v] = ctr[v];
-        ++nfall;
-    }
-    return nfall;
-}
-
-template <int DIR>
-__device__ __forceinline__ int rad_face_flux(double c, double c_hat, bool tau_corr, double tau, const double L[4],
-                                             const double R[4], double G[4])
-{
-    int guard;
-    const Rad4 g = rad_hll_flux(c, c_hat, L[0], L[1], L[2], L[3], R[0], R[1], R[2], R[3], DIR, tau, tau_corr, guard);
-    G[0] = g.e; G[1] = g.x; G[2] = g.y; G[3] = g.z;
-    return guard;
+    return rad_fallback(q, lo, hi);
 }
 
 }  // namespace qk

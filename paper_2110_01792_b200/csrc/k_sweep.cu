@@ -1,25 +1,10 @@
-// k_sweep.cu -- physics policies and launchers of the direction-split sweep path (k_sweep.cuh).
+// k_sweep.cu -- physics policies and launchers of the stencil kernels of an RK stage (k_sweep.cuh) and the
+// flattening-coefficient kernel.
 //
-// Hydro stage:  prim (cons -> rho, v, P, all cells)  ->  chi (flattening, H6)
-//   -> x sweep (D = dFx) -> y sweep (D += dFy) -> z sweep (U' = RK(U, (dFx+dFy)+dFz)).
-// Radiation stage:  rad prim (E_r, f = F_r/(c E_r))  -> x, y, z sweeps the same way.
-#include <stdlib.h>
-
+// Hydro stage:  chi (flattening, H6) -> x sweep (D = dFx) -> y sweep (D += dFy) -> z sweep
+// (U' = RK(U, D + dFz)).  Radiation stage:  x, y, z sweeps, same code with the radiation policy.
 #include "k_sweep.cuh"
 #include "qk_fastmath.cuh"
-
-#ifndef QK_BLX_H
-#define QK_BLX_H 1
-#endif
-#ifndef QK_BLM_H
-#define QK_BLM_H 0
-#endif
-#ifndef QK_BLX_R
-#define QK_BLX_R 1
-#endif
-#ifndef QK_BLM_R
-#define QK_BLM_R 1
-#endif
 
 namespace qk {
 
@@ -46,20 +31,21 @@ __device__ __noinline__ Rad4 rad_hll_flux_slow(double c, double c_hat, double EL
 // RECON: 0 = PPM, 1 = PLM with the MC limiter
 template <int RECON>
 struct HydroPhT {
-    static constexpr int NV = 5;
+    static constexpr int NV = 5, NSRC = 6;
     static constexpr bool COUNTS = false;
     // select-only PPM limiter (same values): measured faster in the x sweep, slower in the marching sweeps
-    static constexpr int BL_X = QK_BLX_H, BL_MARCH = QK_BLM_H;
-    static constexpr bool CARRY = true;    // marching sweeps carry the raw interface value (measured: -1.5 %)   // 0 branches, 1 selects, 2 selects in lockstep
+    static constexpr int BL_X = 1, BL_MARCH = 0;
+    static constexpr bool CARRY = true;    // marching sweeps carry the raw interface value (measured: -1.5 %)
+    static constexpr int X_MINB = 5, Y_MINB = 4, Z_MINB = 3;
     const double *w[5];        // rho, vx, vy, vz, P (ghost cells included)
     const double *chi;         // flattening coefficient of the cells -1..n
     double gamma;
     __device__ __forceinline__ double ld(int v, int cidx) const { return __ldg(w[v] + cidx); }
     __device__ __forceinline__ double aux(int cidx) const { return __ldg(chi + cidx); }
     // x sweep: staged sources 0..4 = W, 5 = chi
-    __device__ __forceinline__ const double *src(int s) const { return s < 5 ? w[s] : chi; }
-    __device__ __forceinline__ double win(int v, const double (*buf)[SW_XSEG], int p) const { return buf[v][p]; }
-    __device__ __forceinline__ double win_aux(const double (*buf)[SW_XSEG], int p) const { return buf[5][p]; }
+    __device__ __forceinline__ const double *src(int q) const { return q < 5 ? w[q] : chi; }
+    __device__ __forceinline__ double win(int v, const double (*buf)[SW_XCOLS], int p) const { return buf[v][p]; }
+    __device__ __forceinline__ double win_aux(const double (*buf)[SW_XCOLS], int p) const { return buf[5][p]; }
     template <int BL, class Q>
     __device__ __forceinline__ int states(Q q, double x, double lo[5], double hi[5]) const
     {
@@ -91,9 +77,8 @@ struct HydroPhT {
         }
         return 0;
     }
-    // MODE 2 epilogue: primitives of the updated cell for the next stage's sweeps and,
-    // after the last stage, the cell's CFL signal speed |v| + c_s (eq 21), same operations as
-    // prim_kernel / cfl_max_speed_kernel.
+    // z epilogue: primitives of the updated cell for the next stage's sweeps and, after the last
+    // stage, the cell's CFL signal speed |v| + c_s (eq 21), same operations as prim_kernel / cfl_max_speed_kernel
     struct Tail { double smax = 0.0; int bad = 0; };
     __device__ __forceinline__ void finish(int cidx, const double u[5], const FieldsRW<5> &wout, bool last, Tail &t) const
     {
@@ -127,27 +112,24 @@ struct HydroPhT {
     template <int DIR>
     __device__ __forceinline__ int flux(const double L[5], const double R[5], double, double, double F[5]) const
     {
-#ifdef QK_PLAIN_DIVSQRT
-        face_flux<DIR>(gamma, L, R, F);
-#else
         constexpr int n = 1 + DIR, t1 = 1 + (DIR + 1) % 3, t2 = 1 + (DIR + 2) % 3;
         unsigned risk = 0;
         Flux5 f = hllc_flux_fast(gamma, L[0], L[n], L[t1], L[t2], L[4], R[0], R[n], R[t1], R[t2], R[4], risk);
         if (risk) f = hllc_flux_slow(gamma, L[0], L[n], L[t1], L[t2], L[4], R[0], R[n], R[t1], R[t2], R[4]);
         F[0] = f.m; F[n] = f.pn; F[t1] = f.pt1; F[t2] = f.pt2; F[4] = f.e;
-#endif
         return 0;
     }
 };
 
 // ---- radiation --------------------------------------------------------------------------------------
-// RECON as for hydro; CL: 0 = Levermore closure (eq 23-25), 1 = Eddington approximation
+// RECON as for hydro; CL: 0 = Levermore closure (eq 23-25), 1 = Eddington approximation, 2 = Minerbo
 template <int RECON, int CL>
 struct RadPhT {
-    static constexpr int NV = 4;
+    static constexpr int NV = 4, NSRC = 6;
     static constexpr bool COUNTS = true;
-    static constexpr int BL_X = QK_BLX_R, BL_MARCH = QK_BLM_R;
+    static constexpr int BL_X = 1, BL_MARCH = 1;
     static constexpr bool CARRY = false;   // measured slower with the select-only limiter (+1.5 %)
+    static constexpr int X_MINB = 5, Y_MINB = 4, Z_MINB = 3;
     const double *s[4];        // E_r, fx, fy, fz
     const double *rho, *kR;
     double c, c_hat, dx;
@@ -159,53 +141,27 @@ struct RadPhT {
     }
     __device__ __forceinline__ double aux(int) const { return 0.0; }
     // x sweep: staged sources 0..3 = S, 4 = kappa_R, 5 = rho
-    __device__ __forceinline__ const double *src(int i) const { return i < 4 ? s[i] : (i == 4 ? kR : rho); }
-    __device__ __forceinline__ double win(int v, const double (*buf)[SW_XSEG], int p) const
+    __device__ __forceinline__ const double *src(int q) const { return q < 4 ? s[q] : (q == 4 ? kR : rho); }
+    __device__ __forceinline__ double win(int v, const double (*buf)[SW_XCOLS], int p) const
     {
         return v < 4 ? buf[v][p] : buf[4][p] * buf[5][p];
     }
-    __device__ __forceinline__ double win_aux(const double (*)[SW_XSEG], int) const { return 0.0; }
+    __device__ __forceinline__ double win_aux(const double (*)[SW_XCOLS], int) const { return 0.0; }
     template <int BL, class Q>
     __device__ __forceinline__ int states(Q q, double, double lo[4], double hi[4]) const
     {
         if (RECON == 0) return rad_ppm_cell<BL>(q, lo, hi);
         plm_states<4>(q, lo, hi);
-        int nfall = 0;      // first-order fallback per face state, as in rad_ppm_cell
-        double f2 = (lo[1] * lo[1] + lo[2] * lo[2]) + lo[3] * lo[3];
-        if (f2 > 1.0 || !(lo[0] > 0.0)) {
-#pragma unroll
-            for (int v = 0; v < 4; ++v) lo[v] = q(v, 2);
-            ++nfall;
-        }
-        f2 = (hi[1] * hi[1] + hi[2] * hi[2]) + hi[3] * hi[3];
-        if (f2 > 1.0 || !(hi[0] > 0.0)) {
-#pragma unroll
-            for (int v = 0; v < 4; ++v) hi[v] = q(v, 2);
-            ++nfall;
-        }
-        return nfall;
+        return rad_fallback(q, lo, hi);
     }
     template <int BL, class Q>
     __device__ __forceinline__ int states_carry(Q q, double x, double ifc[4], double lo[4], double hi[4]) const
     {
         if (RECON == 1) return states<BL>(q, x, lo, hi);
         ppm_states_carry<BL, 4>(q, ifc, lo, hi);
-        int nfall = 0;      // first-order fallback per face state, as in rad_ppm_cell
-        double f2 = (lo[1] * lo[1] + lo[2] * lo[2]) + lo[3] * lo[3];
-        if (f2 > 1.0 || !(lo[0] > 0.0)) {
-#pragma unroll
-            for (int v = 0; v < 4; ++v) lo[v] = q(v, 2);
-            ++nfall;
-        }
-        f2 = (hi[1] * hi[1] + hi[2] * hi[2]) + hi[3] * hi[3];
-        if (f2 > 1.0 || !(hi[0] > 0.0)) {
-#pragma unroll
-            for (int v = 0; v < 4; ++v) hi[v] = q(v, 2);
-            ++nfall;
-        }
-        return nfall;
+        return rad_fallback(q, lo, hi);
     }
-    // MODE 2 epilogue: (E_r, f = F_r / (c E_r)) of the updated cell, as rad_prim_kernel
+    // z epilogue: (E_r, f = F_r / (c E_r)) of the updated cell, as rad_prim_kernel
     struct Tail { int bad = 0; };
     __device__ __forceinline__ void finish(int cidx, const double r[4], const FieldsRW<4> &sout, bool, Tail &t) const
     {
@@ -226,9 +182,6 @@ struct RadPhT {
     __device__ __forceinline__ int flux(const double L[4], const double R[4], double krL, double krR, double G[4]) const
     {
         const double tau = (0.5 * (krL + krR)) * dx;
-#ifdef QK_PLAIN_DIVSQRT
-        return rad_face_flux<DIR>(c, c_hat, tau_corr != 0, tau, L, R, G);
-#else
         unsigned risk = 0;
         int guard;
         Rad4 g = rad_hll_flux_fast<CL>(c, c_hat, L[0], L[1], L[2], L[3], R[0], R[1], R[2], R[3], DIR, tau, tau_corr != 0,
@@ -237,14 +190,16 @@ struct RadPhT {
                                         tau_corr != 0, &guard);
         G[0] = g.e; G[1] = g.x; G[2] = g.y; G[3] = g.z;
         return guard;
-#endif
     }
 };
 
 // ---- flattening coefficient in two pointwise passes (H6) -------------------------------
+// (A single kernel marching along z -- P, v of a 32 x 8 tile and its halo in a shared plane, chi~_z from a register
+// window, 40 B/cell instead of 89 -- was built and measured slower: 0.42 ms against 0.31 ms at 256^3, one barrier
+// per plane at 16 resident warps.)
 // pass 1: chi~_x, chi~_y, chi~_z of every cell of [-2, n+1]^3 (one evaluation per cell and direction);
 // pass 2: chi = min over the three directions and the -1, 0, +1 neighbours along each, cells [-1, n]^3.
-__global__ void __launch_bounds__(128) chi_dir_kernel(Geom g, double gamma, const double *__restrict__ P,
+__global__ void __launch_bounds__(128) chi_dir_kernel(Geom g, int k0, double gamma, const double *__restrict__ P,
                                                       const double *__restrict__ vx, const double *__restrict__ vy,
                                                       const double *__restrict__ vz, double *__restrict__ cx,
                                                       double *__restrict__ cy, double *__restrict__ cz)
@@ -254,7 +209,7 @@ __global__ void __launch_bounds__(128) chi_dir_kernel(Geom g, double gamma, cons
     const int w = g.nx + 4;
     if (t >= w * (g.ny + 4)) return;
     const int jj = t / w;
-    const int i = t - jj * w - 2, j = jj - 2, k = (int)blockIdx.y - 2;
+    const int i = t - jj * w - 2, j = jj - 2, k = (int)blockIdx.y + k0;
     const int c = g.at(i, j, k), sy = g.sy, sz = g.sz;
     const double P0 = P[c];
     cx[c] = flatten_coeff_1d(gamma, P[c - 2], P[c - 1], P0, P[c + 1], P[c + 2], vx[c - 1], vx[c + 1]);
@@ -262,14 +217,14 @@ __global__ void __launch_bounds__(128) chi_dir_kernel(Geom g, double gamma, cons
     cz[c] = flatten_coeff_1d(gamma, P[c - 2 * sz], P[c - sz], P0, P[c + sz], P[c + 2 * sz], vz[c - sz], vz[c + sz]);
 }
 
-__global__ void __launch_bounds__(128) chi_min_kernel(Geom g, const double *__restrict__ cx, const double *__restrict__ cy,
+__global__ void __launch_bounds__(128) chi_min_kernel(Geom g, int k0, const double *__restrict__ cx, const double *__restrict__ cy,
                                                       const double *__restrict__ cz, double *__restrict__ chi)
 {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     const int w = g.nx + 2;
     if (t >= w * (g.ny + 2)) return;
     const int jj = t / w;
-    const int i = t - jj * w - 1, j = jj - 1, k = (int)blockIdx.y - 1;
+    const int i = t - jj * w - 1, j = jj - 1, k = (int)blockIdx.y + k0;
     const int c = g.at(i, j, k), sy = g.sy, sz = g.sz;
     double x = 1.0;      // same nesting as the oracle: min(1, min(lo, min(mid, hi))) per direction
     x = lesser(x, lesser(cx[c - 1], lesser(cx[c], cx[c + 1])));
@@ -278,25 +233,31 @@ __global__ void __launch_bounds__(128) chi_min_kernel(Geom g, const double *__re
     chi[c] = x;
 }
 
-int launch_chi_two_pass(const Geom &g, double gamma, CHydro5 W, double *cx, double *cy, double *cz, double *chi,
-                        cudaStream_t st)
+// chi~_d for the planes [d0, d1) (within [-2, nz+2)), then chi for the planes [m0, m1) (within [-1, nz+1)); an empty
+// range launches nothing.  The whole box is (-2, nz+2, -1, nz+1); a decomposed box does the planes that need no
+// neighbour data first.
+int launch_chi(const Geom &g, double gamma, CHydro5 W, double *cx, double *cy, double *cz, double *chi, int d0, int d1,
+               int m0, int m1, cudaStream_t st)
 {
-    dim3 g1(((g.nx + 4) * (g.ny + 4) + 127) / 128, g.nz + 4), g2(((g.nx + 2) * (g.ny + 2) + 127) / 128, g.nz + 2);
-    chi_dir_kernel<<<g1, 128, 0, st>>>(g, gamma, W.E, W.mx, W.my, W.mz, cx, cy, cz);
-    chi_min_kernel<<<g2, 128, 0, st>>>(g, cx, cy, cz, chi);
-    return 2;
+    int n = 0;
+    if (d1 > d0) {
+        dim3 g1(((g.nx + 4) * (g.ny + 4) + 127) / 128, d1 - d0);
+        chi_dir_kernel<<<g1, 128, 0, st>>>(g, d0, gamma, W.E, W.mx, W.my, W.mz, cx, cy, cz);
+        ++n;
+    }
+    if (m1 > m0) {
+        dim3 g2(((g.nx + 2) * (g.ny + 2) + 127) / 128, m1 - m0);
+        chi_min_kernel<<<g2, 128, 0, st>>>(g, m0, cx, cy, cz, chi);
+        ++n;
+    }
+    return n;
 }
 
+// marching chunk: 32 cells, shorter for small boxes so that ~8 waves of warps stay available on 148 SMs x 16 warps
 static int sweep_len(int n_m, long long columns)
 {
-    static int forced = -1;
-    if (forced < 0) {
-        const char *e = getenv("QK_SWEEP_LEN");
-        forced = e ? atoi(e) : 0;
-    }
-    int len = forced > 0 ? forced : 32;
-    // keep at least ~8 waves of warps on 148 SMs x 16 warps
-    while (forced <= 0 && len > 8 && columns / 32 * ((n_m + len - 1) / len) < 148LL * 16 * 8) len /= 2;
+    int len = 32;
+    while (len > 8 && columns / 32 * ((n_m + len - 1) / len) < 148LL * 16 * 8) len /= 2;
     if (len > n_m) len = n_m;
     return len < 1 ? 1 : len;
 }
@@ -304,35 +265,37 @@ static int sweep_len(int n_m, long long columns)
 template <class PH>
 static int launch_sweeps(const PH &ph, const Geom &g, double dtdx, int stage, FieldsRW<PH::NV> D, FieldsRO<PH::NV> U,
                          FieldsRO<PH::NV> U0, FieldsRW<PH::NV> out, FieldsRW<PH::NV> pout, Counters *ctr,
-                         StateCache *cache, cudaStream_t st, int which, const double *dtdx_dev = nullptr)
+                         StateCache *cache, cudaStream_t st, int which, const double *dtdx_dev, int k0, int k1)
 {
     const RkArgs rk{dtdx, stage, dtdx_dev};
     int n = 0;
-    if (which & 1) {
-        constexpr int rows = SW_XROWS * SW_XNROW;
-        dim3 grid((g.nx + SW_XW - 1) / SW_XW, (g.ny + rows - 1) / rows, g.nz), block(32, SW_XROWS);
-        sweep_x_kernel<PH><<<grid, block, 0, st>>>(ph, g, D, ctr);
+    if ((which & 1) && k1 > k0) {        // x sweep of the planes [k0, k1)
+        constexpr int rows = SW_XYWARPS * SW_XNROW;
+        dim3 grid((g.nx + SW_XW - 1) / SW_XW, (g.ny + rows - 1) / rows, k1 - k0);
+        sweep_x_kernel<PH><<<grid, SW_NT, 0, st>>>(ph, g, k0, D, ctr);
         ++n;
     }
     const int bx = (g.nx + SW_NT - 1) / SW_NT;
-    if (which & 2) {
+    if ((which & 2) && k1 > k0) {        // y sweep of the planes [k0, k1)
         const int len = sweep_len(g.ny, (long long)g.nx * g.nz);
-        dim3 grid(bx, g.nz, (g.ny + len - 1) / len);
-        sweep_march_kernel<PH, 1, 1><<<grid, SW_NT, 0, st>>>(ph, g, len, D, rk, U, U0, out, pout, ctr, cache);
+        dim3 grid(bx, k1 - k0, (g.ny + len - 1) / len);
+        sweep_march_kernel<PH, 1><<<grid, SW_NT, 0, st>>>(ph, g, len, k0, D, rk, U, U0, out, pout, ctr, cache);
         ++n;
     }
-    if (which & 4) {
+    if (which & 4) {                     // z sweep: always the whole box
         const int len = sweep_len(g.nz, (long long)g.nx * g.ny);
         dim3 grid(bx, g.ny, (g.nz + len - 1) / len);
-        sweep_march_kernel<PH, 2, 2><<<grid, SW_NT, 0, st>>>(ph, g, len, D, rk, U, U0, out, pout, ctr, cache);
+        sweep_march_kernel<PH, 2><<<grid, SW_NT, 0, st>>>(ph, g, len, 0, D, rk, U, U0, out, pout, ctr, cache);
         ++n;
     }
     return n;
 }
 
+// `which`: bit 0 = x sweep (D = dF_x), bit 1 = y sweep (D += dF_y), bit 2 = z sweep (RK stage update); x and y
+// sweeps cover the planes [k0, k1)
 int launch_hydro_sweeps(const Geom &g, double gamma, unsigned scheme, double dtdx, int stage, CHydro5 W,
                         const double *chi, Hydro5 D, CHydro5 U, CHydro5 U0, Hydro5 out, Hydro5 Wout, Counters *ctr,
-                        StateCache *cache, cudaStream_t st, int which, const double *dtdx_dev)
+                        StateCache *cache, cudaStream_t st, int which, const double *dtdx_dev, int k0, int k1)
 {
     FieldsRW<5> d{{D.rho, D.mx, D.my, D.mz, D.E}}, o{{out.rho, out.mx, out.my, out.mz, out.E}};
     FieldsRO<5> u{{U.rho, U.mx, U.my, U.mz, U.E}}, u0{{U0.rho, U0.mx, U0.my, U0.mz, U0.E}};
@@ -340,14 +303,14 @@ int launch_hydro_sweeps(const Geom &g, double gamma, unsigned scheme, double dtd
     auto go = [&](auto ph) {
         ph.w[0] = W.rho; ph.w[1] = W.mx; ph.w[2] = W.my; ph.w[3] = W.mz; ph.w[4] = W.E;
         ph.chi = chi; ph.gamma = gamma;
-        return launch_sweeps(ph, g, dtdx, stage, d, u, u0, o, wo, ctr, cache, st, which, dtdx_dev);
+        return launch_sweeps(ph, g, dtdx, stage, d, u, u0, o, wo, ctr, cache, st, which, dtdx_dev, k0, k1);
     };
     return (scheme & QK_FLAG_PLM) ? go(HydroPhT<1>()) : go(HydroPhT<0>());
 }
 
 int launch_rad_sweeps(const Geom &g, const PhysConsts &pc, double dtdx, int stage, CRad4p S, const double *rho,
                       const double *kappaR, Rad4p D, CRad4p R, CRad4p R0, Rad4p out, Rad4p Sout, Counters *ctr,
-                      cudaStream_t st, int which)
+                      cudaStream_t st, int which, const double *dtdx_dev, int k0, int k1)
 {
     FieldsRW<4> d{{D.E, D.Fx, D.Fy, D.Fz}}, o{{out.E, out.Fx, out.Fy, out.Fz}};
     FieldsRO<4> u{{R.E, R.Fx, R.Fy, R.Fz}}, u0{{R0.E, R0.Fx, R0.Fy, R0.Fz}};
@@ -356,12 +319,62 @@ int launch_rad_sweeps(const Geom &g, const PhysConsts &pc, double dtdx, int stag
         ph.s[0] = S.E; ph.s[1] = S.Fx; ph.s[2] = S.Fy; ph.s[3] = S.Fz;
         ph.rho = rho; ph.kR = kappaR;
         ph.c = pc.c; ph.c_hat = pc.c_hat; ph.dx = pc.dx; ph.tau_corr = (pc.flags & QK_FLAG_TAU_CORR) ? 1 : 0;
-        return launch_sweeps(ph, g, dtdx, stage, d, u, u0, o, so, ctr, nullptr, st, which);
+        return launch_sweeps(ph, g, dtdx, stage, d, u, u0, o, so, ctr, nullptr, st, which, dtdx_dev, k0, k1);
     };
     const bool plm = (pc.flags & QK_FLAG_PLM) != 0;
     const int cl = (pc.flags & QK_FLAG_EDDINGTON) ? 1 : ((pc.flags & QK_FLAG_MINERBO) ? 2 : 0);
     if (plm) return cl == 1 ? go(RadPhT<1, 1>()) : (cl == 2 ? go(RadPhT<1, 2>()) : go(RadPhT<1, 0>()));
     return cl == 1 ? go(RadPhT<0, 1>()) : (cl == 2 ? go(RadPhT<0, 2>()) : go(RadPhT<0, 0>()));
+}
+
+// ---- reconstruction variables of a whole field set (all cells, ghosts included): only when no kernel has left
+// them next to the state -- after qk_set_state / qk_set_raw, and every stage with Dirichlet faces, whose ghost
+// cells hold caller-supplied conserved values ---------------------------------------------------------------
+__global__ void __launch_bounds__(256) prim_kernel(Geom g, double gamma, CHydro5 U, Hydro5 W, Counters *ctr)
+{
+    int bad = 0;
+    for (int cidx = blockIdx.x * blockDim.x + threadIdx.x; cidx < g.ntot; cidx += gridDim.x * blockDim.x) {
+        const Prim w = cons_to_prim(gamma, U.rho[cidx], U.mx[cidx], U.my[cidx], U.mz[cidx], U.E[cidx]);
+        W.rho[cidx] = w.rho; W.mx[cidx] = w.vx; W.my[cidx] = w.vy; W.mz[cidx] = w.vz; W.E[cidx] = w.P;
+        if (!(w.rho > 0.0) || !(w.P > 0.0)) {   // only interior cells count (their ghost images would double count)
+            const int kk = cidx / g.sz, rem = cidx - kk * g.sz, jj = rem / g.sy, ii = rem - jj * g.sy;
+            if (ii >= NG && ii < NG + g.nx && jj >= NG && jj < NG + g.ny && kk >= NG && kk < NG + g.nz) ++bad;
+        }
+    }
+    if (bad) atomicAdd((unsigned long long *)&ctr->bad_state, (unsigned long long)bad);
+}
+
+__global__ void __launch_bounds__(256) rad_prim_kernel(Geom g, double c, CRad4p R, Rad4p S, Counters *ctr)
+{
+    int bad = 0;
+    for (int cidx = blockIdx.x * blockDim.x + threadIdx.x; cidx < g.ntot; cidx += gridDim.x * blockDim.x) {
+        const double E = R.E[cidx], cE = c * E;
+        S.E[cidx] = E;
+        S.Fx[cidx] = R.Fx[cidx] / cE;
+        S.Fy[cidx] = R.Fy[cidx] / cE;
+        S.Fz[cidx] = R.Fz[cidx] / cE;
+        if (!(E > 0.0)) {
+            const int kk = cidx / g.sz, rem = cidx - kk * g.sz, jj = rem / g.sy, ii = rem - jj * g.sy;
+            if (ii >= NG && ii < NG + g.nx && jj >= NG && jj < NG + g.ny && kk >= NG && kk < NG + g.nz) ++bad;
+        }
+    }
+    if (bad) atomicAdd((unsigned long long *)&ctr->bad_state, (unsigned long long)bad);
+}
+
+int launch_prim(const Geom &g, double gamma, CHydro5 U, Hydro5 W, Counters *ctr, cudaStream_t st)
+{
+    int blocks = (g.ntot + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    prim_kernel<<<blocks, 256, 0, st>>>(g, gamma, U, W, ctr);
+    return 1;
+}
+
+int launch_rad_prim(const Geom &g, double c, CRad4p R, Rad4p S, Counters *ctr, cudaStream_t st)
+{
+    int blocks = (g.ntot + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    rad_prim_kernel<<<blocks, 256, 0, st>>>(g, c, R, S, ctr);
+    return 1;
 }
 
 }  // namespace qk

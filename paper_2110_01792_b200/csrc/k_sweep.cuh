@@ -1,53 +1,42 @@
-// k_sweep.cuh -- direction-split, barrier-free sweep kernels shared by the hydro and radiation stages.
+// k_sweep.cuh -- the two stencil kernels of an RK stage, shared by the hydro and the radiation policy (k_sweep.cu).
 //
-// The stage kernels are bound by the latency of the fp64 pipe rather than by HBM (a stage
-// moves ~530 B/cell, 1.4 ms of HBM time, against 2.7 ms measured).  The sweeps trade a few hundred bytes per
-// cell of extra traffic for instruction streams that never wait on another warp:
+// The sweeps read the RECONSTRUCTION variables of the stage's state -- primitives W = (rho, v, P), or
+// S = (E_r, f = F_r/(c E_r)), PAPER.md:178 -- which the kernel that produced the state wrote next to it (z sweep,
+// exchange); no face flux ever exists in HBM, only the running flux difference D:
 //
-//   sweep_x_kernel     : one thread per cell, one warp per 30-cell x segment walking 8 rows, row segments
-//                        staged global -> shared by cp.async one row ahead.  Lane l owns cell
-//                        30 b - 1 + l; the high face state of the left neighbour and the flux of the
-//                        right neighbour arrive by warp shuffle, so lanes 1..30 produce a flux
-//                        difference and lanes 0, 31 are halo lanes.  Writes D = dF_x.
-//   sweep_march_kernel : one thread per (x, other) column, marching along y or z over a chunk of
-//                        cells.  The five-cell reconstruction window of the column lives in a
-//                        thread-private shared-memory ring (no __syncthreads anywhere); the high face
-//                        state and the low-face flux of the previous cell stay in registers.
-//                        MODE 1 (y): D = D + dF_y.   MODE 2 (z): out = RK stage update with
-//                        (D + dF_z), i.e. the paper's sum order ((dFx + dFy) + dFz), plus
-//                        the policy's `finish` epilogue: the reconstruction variables of the updated
-//                        cell for the next stage and, after the last stage, its CFL speed.
+//   sweep_x_kernel     : one warp per 30-cell x segment walking 8 rows; row segments staged global -> shared by
+//                        16-byte cp.async one row ahead, converted by the staging lanes; both face states of the
+//                        lane's cell, left neighbour's high state and right neighbour's flux by warp shuffle.
+//                        Writes D = dF_x.
+//   sweep_march_kernel : one thread per (x, other) column marching along y or z over a chunk of cells; the
+//                        five-cell window of the column lives in a thread-private shared-memory ring (no barrier
+//                        anywhere), the high face state, the low-face flux and the raw eq 22 interface value of
+//                        the previous cell stay in registers.  y: D += dF_y.  z: RK stage update
+//                        with (dF_x + dF_y) + dF_z (the paper's sum order) and, after the last hydro
+//                        stage, the CFL signal speed of the new state (eq 21).
 //
-// `PH` is the physics policy (k_sweep.cu): NV reconstructed variables, SW_NR window variables per
-// cell (the last one may be a face auxiliary such as kappa_R rho), `states` = limited face states of
-// one cell, `flux<DIR>` = Riemann flux through a face.  Each face state / face of the grid is counted
-// by exactly one thread for the integer diagnostics (same convention as the oracle: states of the
-// cells -1..n and faces 0..n of the sweep direction, other two indices interior).
+// HBM traffic per cell and stage (hydro): x reads W + chi (48 B), writes D (40); y reads W + chi + D (88), writes D
+// (40); z reads W + chi + D + U (128) + U^n in stage 2 (40), writes the new state and its primitives (80): 424-464 B
+// with the flattening kernel's 40.  Two leaner layouts were built and measured slower: reading
+// the conserved state and converting every loaded cell (no W arrays, 80 B less, +20 % time: the division chains of
+// cons -> prim run 4 x per cell instead of once), and one fused x+y kernel that writes D once (128 B less, +50 % time
+// at 168 registers / 3 warps per scheduler).
+//
+// `PH` is the physics policy: NV reconstructed variables, SW_NR window variables per cell (the last one may be a
+// face auxiliary such as kappa_R rho), `states` = limited face states of one cell, `flux<DIR>` = Riemann flux through a face.  Each face state / face of the grid is counted by exactly
+// one thread for the integer diagnostics (same convention as the oracle: states of the cells -1..n and faces
+// 0..n of the sweep direction, other two indices interior).
 #pragma once
 
-#include "k_stage_common.cuh"
+#include "k_recon.cuh"
 
 namespace qk {
 
-#ifndef QK_SW_NT
-#define QK_SW_NT 128
-#endif
-#ifndef QK_SW_MINB1
-#define QK_SW_MINB1 4
-#endif
-#ifndef QK_SW_MINB2
-#define QK_SW_MINB2 3
-#endif
-#ifndef QK_SW_XROWS
-#define QK_SW_XROWS 4
-#endif
-#ifndef QK_SW_XMINB
-#define QK_SW_XMINB 5
-#endif
-constexpr int SW_NT = QK_SW_NT;       // threads per CTA of the marching kernels (lanes along x)
-constexpr int SW_NR = 5;              // variables per cell kept in the marching window
-constexpr int SW_XW = 30;             // cells updated per warp in the x sweep
-constexpr int SW_XROWS = QK_SW_XROWS; // rows (warps) per CTA in the x sweep
+constexpr int SW_NT = 128;            // threads per CTA: z march = 128 columns along x; xy kernel = 4 warps
+constexpr int SW_NR = 5;              // window variables per cell
+constexpr int SW_XW = 30;             // cells updated per warp row in the xy kernel (lanes 1..30; 0 and 31 are halo lanes)
+constexpr int SW_XCOLS = 38;          // staged columns per warp row: cells i0-4 .. i0+33 (16-byte aligned start)
+constexpr int SW_XYWARPS = SW_NT / 32;
 
 template <int NV> struct FieldsRW { double *f[NV]; };
 template <int NV> struct FieldsRO { const double *f[NV]; };
@@ -55,32 +44,36 @@ template <int NV> struct FieldsRO { const double *f[NV]; };
 // dtdx_dev != nullptr: dt/dx is read from device memory (qk_hydro_step_cfl: the timestep never visits the host)
 struct RkArgs { double dtdx; int stage; const double *dtdx_dev; };
 
-__device__ __forceinline__ void sweep_count(Counters *ctr, int nfall, int nguard)
+__device__ __forceinline__ void sweep_count(Counters *ctr, int nfall, int nguard, int nbad)
 {
     for (int off = 16; off > 0; off >>= 1) {
         nfall += __shfl_xor_sync(0xffffffffu, nfall, off);
         nguard += __shfl_xor_sync(0xffffffffu, nguard, off);
+        nbad += __shfl_xor_sync(0xffffffffu, nbad, off);
     }
     if ((threadIdx.x & 31) == 0) {
         if (nfall) atomicAdd((unsigned long long *)&ctr->fallback, (unsigned long long)nfall);
         if (nguard) atomicAdd((unsigned long long *)&ctr->guard, (unsigned long long)nguard);
+        if (nbad) atomicAdd((unsigned long long *)&ctr->bad_state, (unsigned long long)nbad);
     }
 }
 
-// ---- x sweep -------------------------------------------------------------------------------------------
-// Each warp owns one 30-cell x segment and walks SW_XNROW consecutive rows of it.  The 36-cell row
-// segment of every source array the stencils of its 32 lanes touch is copied global -> shared with
-// cp.async (no register staging), one row ahead of the arithmetic, into a warp-private double buffer:
-// the copy of row r+1 overlaps the PPM / Riemann work of row r and the only synchronisation is
-// __syncwarp.  (Loading the stencils straight from global memory exposed one full memory latency per
-// variable: 45 % of the stall samples, profiles/r1_hydro_ncu.md.)
-#ifndef QK_SW_XNROW
-#define QK_SW_XNROW 8
-#endif
-constexpr int SW_XNROW = QK_SW_XNROW;   // rows walked by one warp
-constexpr int SW_XSEG = SW_XW + 6;      // staged cells per row: lanes' cells -1..30 plus the +-2 stencil halo
-constexpr int SW_NSRC = 6;              // source arrays per policy (window variables are built from them)
+// ---- x sweep ---------------------------------------------------------------------------------------------
+// One warp per 30-cell x segment, walking SW_XNROW consecutive rows.  Lane l owns cell i = i0 - 1 + l (lanes 0
+// and 31 are halo lanes); the 38 cells i0-4 .. i0+33 of a row are staged as 19 pairs: lane l < 19 copies the
+// pair (i0 - 4 + 2l, +1) of every source array global -> shared with one 16-byte cp.async (every row of every
+// field starts 32-byte aligned and i0 is even, so with an even row pitch no pair straddles a 16-byte boundary;
+// odd pitches fall back to two 8-byte copies), one row ahead of the arithmetic, into a warp-private double
+// buffer: no register staging, the copy of row r+1 overlaps the PPM / Riemann work of row r.  Every lane
+// reconstructs both face states of its cell, the left neighbour's high state and the right neighbour's flux
+// arrive by shuffle, and lanes 1..30 write D = dF_x.  Only __syncwarp.
+constexpr int SW_XNROW = 8;             // rows walked by one warp
 
+__device__ __forceinline__ void cp_async16(double *smem_dst, const double *gsrc)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gsrc)
+                 : "memory");
+}
 __device__ __forceinline__ void cp_async8(double *smem_dst, const double *gsrc)
 {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gsrc)
@@ -90,76 +83,85 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 template <class PH>
-__global__ void __launch_bounds__(32 * SW_XROWS, QK_SW_XMINB) sweep_x_kernel(PH ph, Geom g, FieldsRW<PH::NV> D, Counters *ctr)
+__global__ void __launch_bounds__(SW_NT, PH::X_MINB) sweep_x_kernel(PH ph, Geom g, int k0, FieldsRW<PH::NV> D, Counters *ctr)
 {
-    constexpr int NV = PH::NV;
+    constexpr int NV = PH::NV, NSRC = PH::NSRC;
     constexpr unsigned FULL = 0xffffffffu;
-    __shared__ double stage[SW_XROWS][2][SW_NSRC][SW_XSEG];
-    const int lane = threadIdx.x, wy = threadIdx.y;
-    const int k = blockIdx.z;
-    const int j0 = ((int)blockIdx.y * SW_XROWS + wy) * SW_XNROW;
+    __shared__ __align__(16) double stage_all[SW_XYWARPS][2][NSRC][SW_XCOLS];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int k = (int)blockIdx.z + k0;                       // the launch covers the planes k0 .. k0 + gridDim.z - 1
+    const int j0 = ((int)blockIdx.y * SW_XYWARPS + wid) * SW_XNROW;
     const int i0 = (int)blockIdx.x * SW_XW;
-    const int i = i0 - 1 + lane;                              // this lane's cell
-    int nfall = 0, nguard = 0;
     const int nrow = min(SW_XNROW, g.ny - j0);                // warp-uniform; <= 0 for warps past the last row
+    if (nrow <= 0) return;                                    // there is no CTA-wide barrier
+    double(*stage)[NSRC][SW_XCOLS] = stage_all[wid];
+    const int i = i0 - 1 + lane;                              // own cell
+    const int col = lane + 3;                                 // its staged column
+    const bool owner = lane >= 1 && lane <= SW_XW && i < g.nx;      // lanes that store and count
+    const int xi = min(i, g.nx);
+    const bool stager = lane < SW_XCOLS / 2;
+    // the last pairs of the last warp of a row may lie beyond the array: clamp (those columns feed no stored result)
+    const int xs = min(i0 - NG + 2 * lane, g.nx + NG - 2);
+    const bool vec = (g.sy & 1) == 0;
+    int nfall = 0, nguard = 0;
 
-    // cells staged by this lane: i0-3+lane, and for lanes 0..3 also i0+29+lane (clamped into the array)
-    const int ia = min(i0 - 3 + lane, g.nx + NG - 1), ib = min(i0 + 29 + lane, g.nx + NG - 1);
     auto issue = [&](int r) {
-        const int rowbase = g.at(0, j0 + r, k);
-        double(*buf)[SW_XSEG] = stage[wy][r & 1];
+        if (stager) {
+            const int src = g.at(xs, j0 + r, k);
 #pragma unroll
-        for (int sidx = 0; sidx < SW_NSRC; ++sidx) {
-            const double *src = ph.src(sidx) + rowbase;
-            cp_async8(&buf[sidx][lane], src + ia);
-            if (lane < SW_XSEG - 32) cp_async8(&buf[sidx][32 + lane], src + ib);
+            for (int q = 0; q < NSRC; ++q) {
+                const double *p = ph.src(q) + src;
+                double *d = &stage[r & 1][q][2 * lane];
+                if (vec) cp_async16(d, p);
+                else { cp_async8(d, p); cp_async8(d + 1, p + 1); }
+            }
         }
         cp_async_commit();
     };
-    if (nrow > 0) issue(0);
+    issue(0);
     for (int r = 0; r < nrow; ++r) {
         if (r + 1 < nrow) { issue(r + 1); cp_async_wait<1>(); }
         else              { cp_async_wait<0>(); }
         __syncwarp();
-        const double(*buf)[SW_XSEG] = stage[wy][r & 1];
-        const int cidx = g.at(min(i, g.nx), j0 + r, k);      // lanes beyond cell n are not stored, not counted
+        const double(*buf)[SW_XCOLS] = stage[r & 1];
+        const int cidx = g.at(xi, j0 + r, k);
         double lo[NV], hi[NV], L[NV], F[NV];
-        const int nf = ph.template states<PH::BL_X>([&](int v, int m) { return ph.win(v, buf, lane + m); },
-                                                     ph.win_aux(buf, lane + 2), lo, hi);
+        const int nf = ph.template states<PH::BL_X>([&](int v, int q) { return ph.win(v, buf, col - 2 + q); },
+                                                     ph.win_aux(buf, col), lo, hi);
 #pragma unroll
         for (int v = 0; v < NV; ++v) L[v] = __shfl_up_sync(FULL, hi[v], 1);
-        const int gd = ph.template flux<0>(L, lo, ph.win(SW_NR - 1, buf, lane + 1), ph.win(SW_NR - 1, buf, lane + 2), F);   // face i-1/2
-        const bool interior = lane >= 1 && lane <= SW_XW && i < g.nx;
+        const int gd = ph.template flux<0>(L, lo, ph.win(SW_NR - 1, buf, col - 1), ph.win(SW_NR - 1, buf, col), F);   // face i-1/2
 #pragma unroll
         for (int v = 0; v < NV; ++v) {
             const double Fh = __shfl_down_sync(FULL, F[v], 1);
-            if (interior) D.f[v][cidx] = Fh - F[v];
+            if (owner) D.f[v][cidx] = Fh - F[v];
         }
         if (PH::COUNTS) {
             const bool last = lane >= 1 && i == g.nx;
-            if (interior || i == -1 || last) nfall += nf;
-            if (interior || last) nguard += gd;
+            if (owner || i == -1 || last) nfall += nf;
+            if (owner || last) nguard += gd;
         }
-        __syncwarp();                                         // all lanes done with buf before it is refilled
+        __syncwarp();                                         // all lanes done with the buffer before it is refilled
     }
-    if (PH::COUNTS) sweep_count(ctr, nfall, nguard);
+    if (PH::COUNTS) sweep_count(ctr, nfall, nguard, 0);
 }
 
-// DIR = 1 (march along y; blockIdx.y = k) or 2 (march along z; blockIdx.y = j)
-template <class PH, int DIR, int MODE>
-__global__ void __launch_bounds__(SW_NT, MODE == 2 ? QK_SW_MINB2 : QK_SW_MINB1) sweep_march_kernel(PH ph, Geom g, int len, FieldsRW<PH::NV> D, RkArgs rk,
-                                                            FieldsRO<PH::NV> U, FieldsRO<PH::NV> U0,
-                                                            FieldsRW<PH::NV> out, FieldsRW<PH::NV> pout, Counters *ctr,
-                                                            StateCache *cache)
+// ---- y and z sweeps: marching columns ----------------------------------------------------------------------
+// DIR = 1: march along y (blockIdx.y = k), D += dF_y.  DIR = 2: march along z (blockIdx.y = j), RK stage update
+// from (dF_x + dF_y) + dF_z (the paper's sum order).
+template <class PH, int DIR>
+__global__ void __launch_bounds__(SW_NT, DIR == 2 ? PH::Z_MINB : PH::Y_MINB) sweep_march_kernel(PH ph, Geom g, int len, int o0, FieldsRW<PH::NV> D, RkArgs rk,
+                                                                   FieldsRO<PH::NV> U, FieldsRO<PH::NV> U0, FieldsRW<PH::NV> out,
+                                                                   FieldsRW<PH::NV> pout, Counters *ctr, StateCache *cache)
 {
     constexpr int NV = PH::NV;
-    const double dtdx = (MODE == 2 && rk.dtdx_dev) ? __ldg(rk.dtdx_dev) : rk.dtdx;
-    typename PH::Tail tail;                             // per-thread reduction state of the MODE 2 epilogue
+    const double dtdx = (DIR == 2 && rk.dtdx_dev) ? __ldg(rk.dtdx_dev) : rk.dtdx;
+    typename PH::Tail tail;                             // per-thread reduction state of the z epilogue
     __shared__ double ring[5 * SW_NR * SW_NT];          // [slot][var][thread], thread-private columns
     const int tid = threadIdx.x;
     const int i = blockIdx.x * SW_NT + tid;
     const bool active = i < g.nx;
-    const int o = blockIdx.y;
+    const int o = (int)blockIdx.y + o0;                 // y sweep: the launch covers the planes o0 .. o0 + gridDim.y - 1
     const int n_m = DIR == 1 ? g.ny : g.nz;
     const int m0 = (int)blockIdx.z * len;
     const int m1 = min(m0 + len, n_m);
@@ -210,7 +212,7 @@ __global__ void __launch_bounds__(SW_NT, MODE == 2 ? QK_SW_MINB2 : QK_SW_MINB1) 
 #pragma unroll
             for (int v = 0; v < NV; ++v) {
                 din[v] = D.f[v][cidx];
-                if (MODE == 2) {
+                if (DIR == 2) {
                     u[v] = U.f[v][cidx];
                     u0[v] = rk.stage == 1 ? U0.f[v][cidx] : 0.0;
                 }
@@ -235,8 +237,8 @@ __global__ void __launch_bounds__(SW_NT, MODE == 2 ? QK_SW_MINB2 : QK_SW_MINB1) 
             double fresh[NV];
 #pragma unroll
             for (int v = 0; v < NV; ++v) {
-                const double div = din[v] + (Fhi[v] - Flo[v]);
-                if (MODE == 1) {
+                const double div = din[v] + (Fhi[v] - Flo[v]);              // dF_x + dF_y, then (dF_x + dF_y) + dF_z
+                if (DIR == 1) {
                     D.f[v][cidx] = div;
                 } else {
                     const double us = u[v] - dtdx * div;
@@ -245,14 +247,14 @@ __global__ void __launch_bounds__(SW_NT, MODE == 2 ? QK_SW_MINB2 : QK_SW_MINB1) 
                 }
             }
             // the reconstruction variables of the updated cell, for the next stage (and its CFL speed)
-            if (MODE == 2) ph.finish(cidx, fresh, pout, rk.stage == 1, tail);
+            if (DIR == 2) ph.finish(cidx, fresh, pout, rk.stage == 1, tail);
         }
 #pragma unroll
         for (int v = 0; v < NV; ++v) { hiP[v] = hi[v]; Flo[v] = Fhi[v]; }
         const int t = r0; r0 = r1; r1 = r2; r2 = r3; r3 = r4; r4 = t;
     }
-    if (PH::COUNTS) sweep_count(ctr, nfall, nguard);
-    if (MODE == 2) ph.finish_block(tail, rk.stage == 1, ctr, cache);
+    if (PH::COUNTS) sweep_count(ctr, nfall, nguard, 0);
+    if (DIR == 2) ph.finish_block(tail, rk.stage == 1, ctr, cache);
 }
 
 }  // namespace qk

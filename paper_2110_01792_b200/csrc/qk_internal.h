@@ -53,20 +53,19 @@ struct StateCache {
 
 // Timestep kept on the device (qk_hydro_step_cfl): eq 21 evaluated from the cached signal speed by a one-thread
 // kernel, read by the z sweeps.  Lives beside StateCache, outside the part that is cleared between RK stages.
-struct DeviceDt { double dt, dtdx; };
+struct DeviceDt { double dt, dtdx, dts, dtsdx; };     // step, step / dx, radiation substep, substep / dx
 int launch_dt_from_cache(const StateCache *cache, DeviceDt *out, double cfl, double dx, double c_hat, int nsub_max,
-                         cudaStream_t st);
+                         int nsub, cudaStream_t st);
 
 // Kernel classes for per-kernel timing (qk_kernel_times) -- one id per __global__ function family.
-enum KClass { K_FILL = 0, K_CFL, K_PRIM, K_FLATTEN, K_HYDRO_FLUX, K_HYDRO_UPDATE, K_HYDRO_STAGE,
-              K_RAD_PRIM, K_RAD_FLUX, K_RAD_UPDATE, K_RAD_STAGE, K_EXCHANGE,
-              K_HYDRO_SWEEP_X, K_HYDRO_SWEEP_Y, K_HYDRO_SWEEP_Z, K_RAD_SWEEP_X, K_RAD_SWEEP_Y, K_RAD_SWEEP_Z,
-              K_NCLASS };
+enum KClass { K_FILL = 0, K_CFL, K_FLATTEN, K_HYDRO_X, K_HYDRO_Y, K_HYDRO_Z, K_RAD_X, K_RAD_Y, K_RAD_Z, K_EXCHANGE, K_OPACITY, K_PRIM, K_HALO, K_NCLASS };
 
 struct PhysConsts {
     double dx, gamma, c_hat, c, a_rad, kB_mu, cfl, newton_tol;
     double opac_kP0, opac_kR0, opac_rho0;   // opacity law (qk_set_opacity_law); opac_rho0 = 0: the fields as set
     int opac_exp;
+    int opac_texp2;        // ... times (T/T0)^(opac_texp2/2) (qk_set_opacity_law_T); 0: no temperature dependence
+    double opac_T0;
     double eos_alpha;      // > 0: E_g = alpha T^4 / 4 in the exchange (eq 55); 0: ideal gas
     int newton_maxit, nsub_max;
     unsigned flags;
@@ -81,51 +80,43 @@ struct CRad4p { const double *E, *Fx, *Fy, *Fz; };
 
 // comp[i] = vector component field i carries (0, 1, 2) or -1 for a scalar: negated in the image cells of a
 // reflecting wall normal to that axis
-struct FillList { double *f[QK_NFIELDS]; signed char comp[QK_NFIELDS]; int n; };
+// fixed_src[i] != nullptr: ghost cells of field i beyond a QK_BC_FIXED face are copied from that array (same cell):
+// how the RK stage buffers get the Dirichlet values the caller stored in the state fields
+struct FillList { double *f[QK_NFIELDS]; const double *fixed_src[QK_NFIELDS]; signed char comp[QK_NFIELDS]; int n; };
 
 // ---- launchers (each enqueues on `st`; returns the number of kernels launched) -----------------
 struct FaceBc { int t[6]; };      // QK_BC_* of the faces x-lo, x-hi, y-lo, y-hi, z-lo, z-hi
-int launch_fill(const Geom &g, const FaceBc &fb, unsigned ext_faces, const FillList &fl, cudaStream_t st);
+// part 0: the whole ghost shell; 1: all but the ghost planes of the inter-rank faces; 2: only those planes
+int launch_fill(const Geom &g, const FaceBc &fb, unsigned ext_faces, int part, const FillList &fl, cudaStream_t st);
+struct PeerList { double *f[QK_NFIELDS]; };      // the neighbour's arrays that correspond to a FillList
+int launch_halo_push(const Geom &g, const Geom &dg, int face_hi, const FillList &fl, const PeerList &dst,
+                     unsigned long long *flag, unsigned long long epoch, cudaStream_t st);
+int launch_halo_wait(const unsigned long long *flag, unsigned long long epoch, cudaStream_t st);
 int launch_halo_copy(const Geom &g, int face_hi, int unpack, const FillList &fl, double *buf, cudaStream_t st);
 int launch_cfl(const Geom &g, double gamma, CHydro5 U, StateCache *cache, cudaStream_t st);
 
-int launch_prim(const Geom &g, double gamma, CHydro5 U, Hydro5 W, Counters *ctr, cudaStream_t st);
-int launch_flatten(const Geom &g, double gamma, CHydro5 W, double *chi, cudaStream_t st);
-int launch_hydro_flux(const Geom &g, double gamma, int dir, CHydro5 W, const double *chi, Hydro5 flux, cudaStream_t st);
-int launch_hydro_update(const Geom &g, double dtdx, int stage, CHydro5 U, CHydro5 U0, CHydro5 fx, CHydro5 fy,
-                        CHydro5 fz, Hydro5 out, cudaStream_t st);
-
-// fused path (k_hydro.cu, k_rad.cu)
-int launch_flatten_march(const Geom &g, double gamma, CHydro5 U, double *chi, cudaStream_t st);
-int launch_hydro_stage(const Geom &g, double gamma, double dtdx, int stage, CHydro5 U, CHydro5 U0, const double *chi,
-                       Hydro5 out, Counters *ctr, cudaStream_t st);
-
-int launch_rad_stage(const Geom &g, const PhysConsts &pc, double dtdx, int stage, CRad4p R, CRad4p R0, const double *rho,
-                     const double *kappaR, Rad4p out, Counters *ctr, cudaStream_t st);
-
-// sweep path (k_sweep.cu); `which` bit 0 = x sweep, bit 1 = y sweep, bit 2 = z sweep + RK update
+// stencil kernels of an RK stage (k_sweep.cu); `which` bit 0 = x sweep (D = dF_x), bit 1 = y sweep (D += dF_y),
+// bit 2 = z sweep (RK update).  W / S: reconstruction variables of the stage's state with their ghost cells filled;
+// U / R: that state (own-cell reads of the update); U0 / R0: the state at the start of the step; Wout / Sout: the
+// reconstruction variables of the updated interior cells.
+int launch_chi(const Geom &g, double gamma, CHydro5 W, double *cx, double *cy, double *cz, double *chi, int d0, int d1,
+               int m0, int m1, cudaStream_t st);
 int launch_hydro_sweeps(const Geom &g, double gamma, unsigned scheme, double dtdx, int stage, CHydro5 W,
                         const double *chi, Hydro5 D, CHydro5 U, CHydro5 U0, Hydro5 out, Hydro5 Wout, Counters *ctr,
-                        StateCache *cache, cudaStream_t st, int which, const double *dtdx_dev);
-int launch_chi_two_pass(const Geom &g, double gamma, CHydro5 W, double *cx, double *cy, double *cz, double *chi,
-                        cudaStream_t st);
+                        StateCache *cache, cudaStream_t st, int which, const double *dtdx_dev, int k0, int k1);
 int launch_rad_sweeps(const Geom &g, const PhysConsts &pc, double dtdx, int stage, CRad4p S, const double *rho,
                       const double *kappaR, Rad4p D, CRad4p R, CRad4p R0, Rad4p out, Rad4p Sout, Counters *ctr,
-                      cudaStream_t st, int which);
-
+                      cudaStream_t st, int which, const double *dtdx_dev, int k0, int k1);
+int launch_prim(const Geom &g, double gamma, CHydro5 U, Hydro5 W, Counters *ctr, cudaStream_t st);
 int launch_rad_prim(const Geom &g, double c, CRad4p R, Rad4p S, Counters *ctr, cudaStream_t st);
-int launch_rad_flux(const Geom &g, const PhysConsts &pc, int dir, CRad4p S, const double *rho, const double *kappaR,
-                    Rad4p flux, Counters *ctr, cudaStream_t st);
-int launch_rad_update(const Geom &g, double dtdx, int stage, CRad4p R, CRad4p R0, CRad4p gx, CRad4p gy, CRad4p gz,
-                      Rad4p out, cudaStream_t st);
 
-int launch_opacity_law(const Geom &g, const double *rho, double *kP, double *kR, double kP0, double kR0, double rho0,
-                       int e, cudaStream_t st);
-int launch_exchange(const Geom &g, const PhysConsts &pc, double dt, const double *rho, double *mx, double *my,
+// opacity law kappa0 (rho/rho0)^e (T/T0)^(texp2/2) of the interior cells from the current state (X14)
+int launch_opacity_law(const Geom &g, const PhysConsts &pc, CHydro5 U, double *kP, double *kR, cudaStream_t st);
+// dt_dev != nullptr: the substep is read from device memory.  The kernel leaves the CFL signal speed of the updated
+// state in `cache` and, when Wout.rho != nullptr, the reconstruction variables W and S of the updated cells
+int launch_exchange(const Geom &g, const PhysConsts &pc, double dt, const double *dt_dev, const double *rho, double *mx, double *my,
                     double *mz, double *E, double *Er, double *Fx, double *Fy, double *Fz, const double *kP,
                     const double *kR, const double *src, Hydro5 Wout, Rad4p Sout, Counters *ctr, StateCache *cache,
                     cudaStream_t st);
-// Wout.rho == nullptr: exchange only; otherwise the kernel also writes the primitives W and the radiation
-// variables S = (E_r, f) of the updated cells and leaves the CFL speed of the new state in `cache`
 
 }  // namespace qk

@@ -281,8 +281,35 @@ QK_HD Rad4 rad_hll_flux(double c, double c_hat, double EL, double fxL, double fy
 // Matter-radiation exchange (eq 26-43)
 // ---------------------------------------------------------------------------------------------
 
+// (T/T0)^(n2/2), integer n2: repeated multiplication, one square root for odd n2, one division for n2 < 0 --
+// no pow(), so the bits are reproducible (X14)
+QK_HD double temperature_power(double T, double T0, int n2)
+{
+    const int a = n2 < 0 ? -n2 : n2;
+    const double q = T / T0;
+    double p = 1.0;
+    for (int m = 0; m < a / 2; ++m) p = p * q;
+    if (a & 1) p = p * sqrt(q);
+    return n2 < 0 ? 1.0 / p : p;
+}
+
+// density part kappa0 (rho/rho0)^e of the opacity law, integer e
+QK_HD void opacity_density_part(double rho, double kP0, double kR0, double rho0, int e, double &kP, double &kR)
+{
+    const double q = e < 0 ? rho0 / rho : rho / rho0;
+    const int n = e < 0 ? -e : e;
+    double kp = kP0, kr = kR0;
+    for (int m = 0; m < n; ++m) { kp = kp * q; kr = kr * q; }
+    kP = kp; kR = kr;
+}
+
 struct ExchangeConsts {
     double c, c_hat, a_rad, kB_mu, gamma, tol;
+    // kappa(rho, T) law (qk_set_opacity_law_T): kappa_P follows the Newton iterate's temperature with the
+    // d kappa_P/dT term of eq 33; kappa_F ~ kappa_R is taken at the updated temperature
+    bool kappa_T;
+    int texp2, opac_exp;
+    double T0, kP0, kR0, rho0;
     double alpha;          // eos_alpha_t3: E_g = alpha T^4 / 4, C_v = alpha T^3 (eq 55)
     bool eos_alpha_t3;
     int maxit;
@@ -291,6 +318,7 @@ struct ExchangeConsts {
 
 // Backward-Euler update of one cell over dt.  In/out: m (gas momentum), E, Er, F.  Returns 0,
 // 4 (Newton cap reached) or 5 (non-positive E_g or E_r afterwards); iters = Newton updates.
+template <bool KT>
 QK_HD int exchange_cell(const ExchangeConsts &k, double dt, double rho, double &mx, double &my, double &mz,
                         double &E, double &Er, double &Fx, double &Fy, double &Fz, double kappaP, double kappaR,
                         double S, int &iters)
@@ -301,7 +329,7 @@ QK_HD int exchange_cell(const ExchangeConsts &k, double dt, double rho, double &
     const double Eg_old = E - Ekin_old;
     const double Er_old = Er;
     const double Etot = Eg_old + c_ratio * (Er_old + S);        // eq 38
-    const double coef = dt * rho * kappaP * k.c_hat;            // dt rho kappa_P c_hat (X1)
+    double coef = dt * rho * kappaP * k.c_hat;                  // dt rho kappa_P c_hat (X1)
     const double Cv_ideal = rho * k.kB_mu / (k.gamma - 1.0);    // volumetric heat capacity (X2)
     double Eg = Eg_old, Erad = Er_old;
     int it = 0;
@@ -317,12 +345,20 @@ QK_HD int exchange_cell(const ExchangeConsts &k, double dt, double rho, double &
         }
         const double T2 = T * T;
         const double T4 = T2 * T2;
+        double dcoef_dT = 0.0;
+        if (KT) {
+            const double kPT = kappaP * temperature_power(T, k.T0, k.texp2);
+            coef = dt * rho * kPT * k.c_hat;
+            const double dkP_dT = (0.5 * (double)k.texp2) * kPT / T;
+            dcoef_dT = dt * rho * dkP_dT * k.c_hat;
+        }
         const double R = coef * (k.a_rad * T4 - Erad);                    // eq 28 (X1)
         const double FG = (Eg - Eg_old) + c_ratio * R;                    // eq 26
         const double FR = (Erad - Er_old) - (R + S);                      // eq 27
         const bool converged = (fabs(FG / Etot) < k.tol) && (fabs(c_ratio * FR / Etot) < k.tol);  // eq 36-37
         if (converged && k.literal_stop) { finished = true; break; }
-        const double dR_dEg = coef * (4.0 * k.a_rad * (T2 * T)) / Cv;     // eq 33, d kappa/dT = 0
+        double dR_dEg = coef * (4.0 * k.a_rad * (T2 * T)) / Cv;           // eq 33 with d kappa/dT = 0
+        if (KT) dR_dEg = (coef * (4.0 * k.a_rad * (T2 * T)) + dcoef_dT * (k.a_rad * T4 - Erad)) / Cv;   // eq 33
         const double dFG_dEg = 1.0 + c_ratio * dR_dEg;                    // eq 29
         const double dFG_dEr = -(c_ratio * coef);                         // eq 30
         const double dFR_dEg = -dR_dEg;                                   // eq 31
@@ -337,7 +373,11 @@ QK_HD int exchange_cell(const ExchangeConsts &k, double dt, double rho, double &
     }
     int rc = finished ? 0 : 4;
     iters = it;
-    // eq 39-41 with kappa_F ~ kappa_R
+    // eq 39-41 with kappa_F ~ kappa_R, at the updated gas temperature
+    if (KT) {
+        const double T = k.eos_alpha_t3 ? sqrt(sqrt(4.0 * Eg / k.alpha)) : Eg / Cv_ideal;
+        kappaR = kappaR * temperature_power(T, k.T0, k.texp2);
+    }
     const double damp = 1.0 + rho * kappaR * k.c_hat * dt;
     const double Fx1 = Fx / damp, Fy1 = Fy / damp, Fz1 = Fz / damp;
     if (k.static_matter) {                                                // PAPER.md:440 (X11)

@@ -3,7 +3,11 @@
 timestep, PAPER.md:574, 604).
 
 Host-side plumbing only: which faces border a neighbour, who the neighbours are, the order of the
-sends and receives, the reduction of dt.  The halo planes themselves are packed / unpacked by
+sends and receives, the reduction of dt.  Two ways to move the halos: `PeerExchange` (the fast path: the library
+writes boundary planes straight into the neighbours' peer-mapped ghost planes on a side stream and overlaps the
+transfer with the interior work of the stage; Python only introduces the ranks to each other once) and
+`SlabExchange` (portable: a callback per ghost fill packs, sends with torch.distributed point-to-point operations
+and unpacks; it is what the CPU tests drive over gloo).  The halo planes themselves are packed / unpacked by
 kernels of the library (qk_halo_pack / qk_halo_unpack) and moved by torch.distributed point-to-point
 operations (NCCL over NVLink on GPUs, gloo on CPU in the tests).  `SlabExchange` works with any
 object that has qk_set_halo_exchange / qk_halo_doubles / qk_halo_pack / qk_halo_unpack and a
@@ -88,7 +92,8 @@ class SlabExchange:
         return self.buffers[nfields]
 
     def _on_fill(self, nfields):
-        # called by the library before every ghost fill; exceptions cannot cross the C frame
+        # called by the library before every ghost fill; exceptions cannot cross the C frame: a non-zero return
+        # makes the step call fail and later step calls return QK_EINVAL until the exchange is attached again
         try:
             send_lo, send_hi, recv_lo, recv_hi = self._bufs(nfields)
             if self.lo is not None:
@@ -102,9 +107,11 @@ class SlabExchange:
                 self.ctx.qk_halo_unpack(FACE_ZHI, recv_hi)
             self.calls += 1
             self.bytes_sent += 8 * nfields * self.per_field * ((self.lo is not None) + (self.hi is not None))
+            return 0
         except BaseException as e:      # noqa: BLE001 -- re-raised by check() on the Python side
             if self.error is None:
                 self.error = e
+            return 1                    # the library aborts the step (QK_EINVAL) instead of running on stale ghosts
 
     def check(self):
         if self.error is not None:
@@ -120,3 +127,40 @@ class SlabExchange:
 
     def detach(self):
         self.ctx.qk_set_halo_exchange(0, None)
+
+
+class PeerExchange:
+    """Peer-mapped halo exchange (qk_halo_export / qk_set_halo_peers): every rank publishes a handle of its storage,
+    picks up its neighbours' handles and attaches them; from then on the stage path never enters Python.
+    `gather(obj) -> list of objects by rank` is how handles cross ranks (torch.distributed.all_gather_object by
+    default); `min_reduce(x) -> float` reduces the timestep."""
+
+    def __init__(self, ctx, rank: int, world: int, periodic: bool, gather=None, min_reduce=None, barrier=None):
+        self.ctx = ctx
+        self.lo, self.hi = neighbours(rank, world, periodic)
+        if gather is None:
+            import torch.distributed as dist
+
+            def gather(obj):
+                out = [None] * dist.get_world_size()
+                dist.all_gather_object(out, obj)
+                return out
+            barrier = barrier or dist.barrier
+        self.min_reduce = min_reduce or TorchTransport().min_over_ranks
+        handles = gather(ctx.qk_halo_export())
+        ctx.qk_set_halo_peers(handles[self.lo] if self.lo is not None else None,
+                              handles[self.hi] if self.hi is not None else None)
+        if barrier is not None:
+            barrier()            # nobody steps before everybody has attached (the arrival counters restart at attach)
+
+    def global_dt(self, local_dt: float) -> float:
+        if local_dt != local_dt:
+            local_dt = float("-inf")
+        dt = self.min_reduce(local_dt)
+        return float("nan") if dt == float("-inf") else dt
+
+    def check(self):
+        pass
+
+    def detach(self):
+        self.ctx.qk_set_halo_peers(None, None)

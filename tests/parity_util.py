@@ -25,10 +25,7 @@ def make_oracle(params, fields):
 
 
 def make_gpu(params, fields, path=None, **kw):
-    ctx = B.from_params(params, fields, **kw)
-    if path is not None:
-        ctx.qk_set_path(path)
-    return ctx
+    return B.from_params(params, fields, **kw)
 
 
 def rel_errors(ref: dict, got: dict, groups=None):
@@ -46,6 +43,14 @@ def assert_parity(ref, got, tol, groups=None, what=""):
     bad = {k: v for k, v in errs.items() if not (v <= tol)}
     assert not bad, "%s: relative max-norm error above %g: %s (all: %s)" % (what, tol, bad, errs)
     return errs
+
+
+def assert_bitwise(ref, got, names, what=""):
+    """every listed field equal bit for bit (+0 == -0 counts as equal, NaN as different): the number of mismatching
+    cells is reported, so 'bit-identical' is asserted, not inferred from a tolerance"""
+    mism = count_mismatch(ref, got, names)
+    assert not any(mism.values()), "%s: cells that differ from the oracle: %s" % (what, mism)
+    return mism
 
 
 def count_mismatch(ref, got, names):

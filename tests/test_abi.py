@@ -22,7 +22,7 @@ def lib():
 def _declared():
     text = open(os.path.join(ROOT, "include", "qk.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(qk_[a-z_0-9]+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b(qk_[A-Za-z_0-9]+)\s*\(", text)))
 
 
 def test_every_declared_symbol_is_exported(lib):
