@@ -257,11 +257,13 @@ def time_e2e(torch, B, I, params, fields, kind, nf, nsteps, barrier, nsub):
     """End to end through the C ABI with HOST (pinned) buffers, two boxes in flight: per step the evolving fields go
     host -> device (qk_set_state_all), the step runs with the device-resident timestep, and the result comes back
     (qk_get_state_all); a box's next step starts from the result it downloaded.  No host synchronisation inside the
-    loop: uploads, steps and downloads of the two boxes overlap on their copy / compute streams.  Returns ms."""
+    loop: each box has its own compute and copy stream, so uploads, steps and downloads of the two boxes overlap (PCIe is
+    full duplex).  Returns ms."""
     ids = list(range(nf))
     boxes = []
     for b in range(2):
-        ctx = B.from_params(params, fields)
+        with torch.cuda.stream(torch.cuda.Stream()):      # a compute stream of its own: the two boxes never wait on each other
+            ctx = B.from_params(params, fields)
         host_in = [torch.from_numpy(np.ascontiguousarray(fields[I.FIELDS[f]])).clone().pin_memory() for f in range(nf)]
         host_out = [torch.empty_like(t).pin_memory() for t in host_in]
         boxes.append([ctx, host_in, host_out])
@@ -316,16 +318,24 @@ def run_workload(torch, B, I, kind, params, fields, steps, warmup, rank, world, 
     nf = {"hydro": 5, "rhd": 9, "rad": 9}[kind]
     cells = params["nx"] * params["ny"] * params["nz"]
     out = {}
-    with B.from_params(params, fields) as ctx:
+    # a decomposed box owns its storage (cudaMalloc): an allocation of its own can be exported to the neighbours
+    with B.from_params(params, fields, torch_storage=not (decompose and world > 1)) as ctx:
         ctx.rad_dt = 0.3 * params["dx"] / params["c_hat"] if params.get("c_hat", 0.0) > 0.0 else None
         ex = None
+        how = ""
         if decompose and world > 1:
-            # one global box of n x n x (world n) cells, rank r owns the z slab r: ghost planes cross ranks by
-            # NCCL send/recv before every stage fill, dt is the minimum over ranks
+            # one global box of n x n x (world n) cells, rank r owns the z slab r: boundary planes go
+            # straight into the neighbours' peer-mapped ghost planes, overlapped with the interior work of the stage; if a
+            # rank cannot attach its peers every rank falls back to the callback exchange (pack, NCCL send/recv, unpack)
             from paper_2110_01792_b200 import decomp as D
-            ex = D.SlabExchange(ctx, rank, world, True, D.TorchTransport())
-        out["parallelism"] = ("z-slab decomposition of one %dx%dx%d box, halo exchange per RK stage (NCCL p2p), "
-                              "global min dt" % (n, n, n * world)) if ex else "1 box per GPU"
+            ex = D.PeerExchange(ctx, rank, world, True)
+            how = "peer-mapped ghost planes over NVLink, pushes overlapped with the interior sweeps"
+            if not ex.ok:
+                log("[rank %d] peer-mapped exchange unavailable (%r): callback exchange" % (rank, ex.error))
+                ex = D.SlabExchange(ctx, rank, world, True, D.TorchTransport())
+                how = "pack / NCCL send-recv / unpack per ghost fill (callback)"
+        out["parallelism"] = ("z-slab decomposition of one %dx%dx%d box, halo exchange per RK stage (%s), global min dt"
+                              % (n, n, n * world, how)) if ex else "1 box per GPU"
         for _ in range(warmup):
             one_step(ctx, kind, ex)
         ctx.set_all(fields)                        # timed steps are steps 1..K of the config
@@ -350,10 +360,11 @@ def run_workload(torch, B, I, kind, params, fields, steps, warmup, rank, world, 
             out["device_dt"] = {"value": world * cells * steps / (ms_d * 1e-3), "unit": UNIT, "ms_per_step": ms_d / steps,
                                 "call": "qk_hydro_step_cfl" if kind == "hydro" else "qk_rhd_step_cfl(%d)" % nsub}
         if ex is not None:
-            out["halo"] = {"exchanges": ex.calls, "bytes_sent_per_rank": ex.bytes_sent}
+            out["halo"] = {"exchange": how, "exchanges": getattr(ex, "calls", None),
+                           "bytes_sent_per_rank": getattr(ex, "bytes_sent", None)}
             ex.detach()
     if e2e and ex is None and kind != "rad":
-        e2e_steps = max(2, min(steps, 6))
+        e2e_steps = max(2, min(steps, 10))
         nsub = max(1, out["info"]["nsub"])
         ms_e = allmax(time_e2e(torch, B, I, params, fields, kind, nf, e2e_steps, barrier, nsub))
         out["e2e"] = {"value": world * cells * e2e_steps / (ms_e * 1e-3), "unit": UNIT,

@@ -199,7 +199,8 @@ int qk_halo_unpack(qk_ctx *ctx, int face, const double *dev_buf);
  *                       rank attaches, and only then does any rank step (the arrival counters restart at attach).  All
  *                       ranks must then make the same sequence of step / fill calls.  Needs nz >= QK_NG, equal nx, ny;
  *                       nz may differ between ranks.  (NULL, NULL) detaches.  qk_cfl_dt stays local: the caller takes
- *                       the minimum over ranks.  The result equals the single-box update bit for bit. */
+ *                       the minimum over ranks.  The result equals the single-box update bit for bit.  QK_EINVAL when
+ *                       the driver has no stream memory operations (use qk_set_halo_exchange then). */
 typedef struct qk_halo_handle {
     unsigned char ipc[64];        /* cudaIpcMemHandle_t of the allocation that holds the storage (has_ipc != 0)    */
     unsigned long long base;      /* device address of the storage in the exporting process                        */

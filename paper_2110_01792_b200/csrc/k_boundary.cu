@@ -171,13 +171,6 @@ __global__ void halo_signal_kernel(unsigned long long *flag, unsigned long long 
     __threadfence_system();
 }
 
-// fallback for drivers without stream memory operations: one thread polls the arrival counter
-__global__ void halo_wait_kernel(const unsigned long long *flag, unsigned long long epoch)
-{
-    while (*(volatile const unsigned long long *)flag < epoch) __nanosleep(200);
-    __threadfence_system();
-}
-
 int launch_halo_push(const Geom &g, const Geom &dg, int face_hi, const FillList &fl, const PeerList &dst,
                      unsigned long long *flag, unsigned long long epoch, cudaStream_t st)
 {
@@ -188,12 +181,6 @@ int launch_halo_push(const Geom &g, const Geom &dg, int face_hi, const FillList 
     halo_push_kernel<<<(unsigned)blocks, 256, 0, st>>>(g, dg, face_hi, fl, dst);
     halo_signal_kernel<<<1, 1, 0, st>>>(flag, epoch);
     return 2;
-}
-
-int launch_halo_wait(const unsigned long long *flag, unsigned long long epoch, cudaStream_t st)
-{
-    halo_wait_kernel<<<1, 1, 0, st>>>(flag, epoch);
-    return 1;
 }
 
 int launch_fill(const Geom &g, const FaceBc &fb, unsigned ext, int part, const FillList &fl, cudaStream_t st)

@@ -185,7 +185,8 @@ CRad4p cr4(double *const *f) { return CRad4p{f[0], f[1], f[2], f[3]}; }
 
 void reset_counters(qk_ctx *c) { cudaMemsetAsync(c->ctr, 0, sizeof(Counters), c->stream); }
 
-// stream memory operation of the driver (cuStreamWaitValue64), fetched once; nullptr: poll with a one-thread kernel
+// stream memory operation of the driver (cuStreamWaitValue64), fetched once; nullptr: not available (then
+// qk_set_halo_peers refuses: a kernel that polls a counter another rank writes must never be launched)
 typedef CUresult (*wait_value_fn)(CUstream, CUdeviceptr, cuuint64_t, unsigned int);
 wait_value_fn stream_wait_value()
 {
@@ -266,9 +267,8 @@ int fill_end(qk_ctx *c)
     int nl = 0;
     for (int side = 0; side < 2; ++side) {
         if (!(c->ext_faces & (side ? QK_FACE_ZHI : QK_FACE_ZLO))) continue;
-        wait_value_fn w = stream_wait_value();
-        if (!w || w((CUstream)c->stream, (CUdeviceptr)(c->arrive + side), (cuuint64_t)c->epoch, 0u /* GEQ */) != CUDA_SUCCESS)
-            nl += launch_halo_wait(c->arrive + side, c->epoch, c->stream);
+        if (stream_wait_value()((CUstream)c->stream, (CUdeviceptr)(c->arrive + side), (cuuint64_t)c->epoch, 0u /* GEQ */) !=
+            CUDA_SUCCESS) { c->halo_failed = true; return QK_ECUDA; }
     }
     nl += launch_fill(c->g, c->fb, c->ext_faces, 2, c->pending, c->stream);
     // the planes just pushed may be overwritten by what follows only once the push has read them
@@ -775,7 +775,7 @@ int qk_set_halo_peers(qk_ctx *c, const qk_halo_handle *lo, const qk_halo_handle 
     c->halo_fn = nullptr;
     c->halo_failed = false;
     if (!lo && !hi) return QK_OK;
-    if (c->g.nz < NG) return QK_EINVAL;
+    if (c->g.nz < NG || !stream_wait_value()) return QK_EINVAL;
     const qk_halo_handle *hs[2] = {lo, hi};
     for (int p = 0; p < 2; ++p) {
         const qk_halo_handle *h = hs[p];

@@ -91,7 +91,6 @@ int launch_fill(const Geom &g, const FaceBc &fb, unsigned ext_faces, int part, c
 struct PeerList { double *f[QK_NFIELDS]; };      // the neighbour's arrays that correspond to a FillList
 int launch_halo_push(const Geom &g, const Geom &dg, int face_hi, const FillList &fl, const PeerList &dst,
                      unsigned long long *flag, unsigned long long epoch, cudaStream_t st);
-int launch_halo_wait(const unsigned long long *flag, unsigned long long epoch, cudaStream_t st);
 int launch_halo_copy(const Geom &g, int face_hi, int unpack, const FillList &fl, double *buf, cudaStream_t st);
 int launch_cfl(const Geom &g, double gamma, CHydro5 U, StateCache *cache, cudaStream_t st);
 

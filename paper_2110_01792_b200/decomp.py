@@ -148,10 +148,22 @@ class PeerExchange:
             barrier = barrier or dist.barrier
         self.min_reduce = min_reduce or TorchTransport().min_over_ranks
         handles = gather(ctx.qk_halo_export())
-        ctx.qk_set_halo_peers(handles[self.lo] if self.lo is not None else None,
-                              handles[self.hi] if self.hi is not None else None)
-        if barrier is not None:
-            barrier()            # nobody steps before everybody has attached (the arrival counters restart at attach)
+        self.error = None
+        try:
+            ctx.qk_set_halo_peers(handles[self.lo] if self.lo is not None else None,
+                                  handles[self.hi] if self.hi is not None else None)
+        except Exception as e:      # e.g. no IPC handle for this kind of allocation, no stream memory operations
+            self.error = e
+        # nobody steps before everybody has attached (the arrival counters restart at attach); the reduction is the
+        # barrier, and if any rank failed every rank detaches so that the caller can fall back to SlabExchange
+        self.ok = self.min_reduce(0.0 if self.error else 1.0) > 0.5
+        if not self.ok:
+            try:
+                ctx.qk_set_halo_peers(None, None)
+            except Exception:
+                pass
+        elif barrier is not None:
+            barrier()
 
     def global_dt(self, local_dt: float) -> float:
         if local_dt != local_dt:

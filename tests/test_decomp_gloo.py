@@ -143,3 +143,111 @@ def test_slab_extents_and_neighbours():
     assert D.neighbours(0, 2, True) == (1, 1) and D.neighbours(1, 2, True) == (0, 0)
     assert D.neighbours(0, 3, False) == (None, 1) and D.neighbours(2, 3, False) == (1, None)
     assert D.neighbours(0, 4, True) == (3, 1)
+
+
+# ------------------------------------------------------------------------------------------------
+# the peer-mapped plan (decomp.PeerExchange): handles cross ranks once, then every rank writes its boundary planes
+# straight into its neighbours' ghost planes and raises their arrival counters.  Stand-in: the "device storage" of a
+# rank is a POSIX shared-memory block, the handle is its name, a push is a numpy copy into the neighbour's block.
+# ------------------------------------------------------------------------------------------------
+class ShmPeerCtx(NumpyCtx):
+    def __init__(self, shape3, nfields, bc, rank):
+        from multiprocessing import shared_memory
+        self.shape3 = shape3
+        n = nfields * int(np.prod(shape3)) + 2
+        self.shm = shared_memory.SharedMemory(create=True, size=8 * n, name="qk_peer_test_%d_%d" % (os.getppid(), rank))
+        flat = np.ndarray((n,), dtype=np.float64, buffer=self.shm.buf)
+        flat[:] = 0.0
+        fields = [flat[f * int(np.prod(shape3)):(f + 1) * int(np.prod(shape3))].reshape(shape3) for f in range(nfields)]
+        self.arrive = flat[-2:]                     # [from lo neighbour, from hi neighbour]
+        super().__init__(fields, bc)
+        self.peers, self.epoch, self.opened = [None, None], 0, []
+
+    def qk_halo_export(self):
+        return (self.shm.name, self.shape3, len(self.f))
+
+    def qk_set_halo_peers(self, lo, hi):
+        from multiprocessing import shared_memory
+        self.faces = 0
+        for side, h in enumerate((lo, hi)):
+            if h is None:
+                continue
+            name, shape3, nf = h
+            shm = shared_memory.SharedMemory(name=name)
+            self.opened.append(shm)
+            flat = np.ndarray((nf * int(np.prod(shape3)) + 2,), dtype=np.float64, buffer=shm.buf)
+            fields = [flat[f * int(np.prod(shape3)):(f + 1) * int(np.prod(shape3))].reshape(shape3) for f in range(nf)]
+            self.peers[side] = (fields, flat[-2:], shape3[0] - 2 * NG)
+            self.faces |= D.FACE_ZHI if side else D.FACE_ZLO
+
+    def fill(self):
+        import time
+        self.epoch += 1
+        for side, p in enumerate(self.peers):
+            if p is None:
+                continue
+            fields, arrive, nz_nb = p
+            for mine, theirs in zip(self.f, fields):
+                if side == 0:       # my low planes -> the low neighbour's HIGH ghost planes
+                    theirs[NG + nz_nb:NG + nz_nb + NG, NG:-NG, NG:-NG] = mine[NG:2 * NG, NG:-NG, NG:-NG]
+                else:               # my high planes -> the high neighbour's LOW ghost planes
+                    theirs[0:NG, NG:-NG, NG:-NG] = mine[self.nz:self.nz + NG, NG:-NG, NG:-NG]
+            arrive[1 if side == 0 else 0] = self.epoch      # I am the HIGH neighbour of my low peer
+        for side, p in enumerate(self.peers):
+            t0 = time.time()
+            while p is not None and self.arrive[side] < self.epoch:
+                assert time.time() - t0 < 60, "peer never arrived"
+                time.sleep(0.001)
+        super().fill()
+
+    def close(self):
+        self.f, self.arrive, self.peers = None, None, None
+        for s in self.opened:
+            s.close()
+        self.shm.close()
+        self.shm.unlink()
+
+
+def _peer_worker(rank, world, port, bc, shape, out):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        import oracle as O
+        nzg, ny, nx = shape
+        rng = np.random.Generator(np.random.PCG64(6))
+        glob = [rng.standard_normal(shape) for _ in range(2)]
+        g = O.Grid(nx, ny, nzg, 1.0 / nx, 5.0 / 3.0, bc=bc)
+        for f, a in enumerate(glob):
+            g.set_state(f, a)
+        g.fill_boundary(O.FILL_HYDRO)
+        ref = [g.get_raw(f) for f in range(2)]
+        g.close()
+        k0, nz = D.slab_extent(nzg, rank, world)
+        ctx = ShmPeerCtx((nz + 2 * NG, ny + 2 * NG, nx + 2 * NG), 2, bc, rank)
+        for f, a in enumerate(glob):
+            ctx.f[f][:] = np.nan
+            ctx.f[f][NG:-NG, NG:-NG, NG:-NG] = a[k0:k0 + nz]
+        ex = D.PeerExchange(ctx, rank, world, periodic=(bc == 0))
+        for _ in range(3):
+            ctx.fill()
+            dist.barrier()          # a rank must not start the next push while a neighbour still reads (on the device the
+                                    # RK stage structure gives this order: DESIGN.md section 8)
+        ok = all(np.array_equal(ctx.f[f], ref[f][k0:k0 + nz + 2 * NG]) for f in range(2))
+        dt = ex.global_dt(1.5 - 0.25 * rank)
+        dist.barrier()
+        ctx.close()
+        out[rank] = (ok, dt)
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world", [2, 3])
+@pytest.mark.parametrize("bc", [0, 1], ids=["periodic", "outflow"])
+def test_peer_exchange_plan_matches_global_fill(world, bc):
+    out = mp.Manager().dict()
+    mp.spawn(_peer_worker, args=(world, _free_port(), bc, (14, 5, 6), out), nprocs=world, join=True)
+    for rank in range(world):
+        ok, dt = out[rank]
+        assert ok, "rank %d: ghost zones differ from the global fill" % rank
+        assert dt == 1.5 - 0.25 * (world - 1)
