@@ -56,10 +56,10 @@ NCU_TRAFFIC_GB_256 = {}     # kernel class -> GB per launch, read from profiles/
 
 
 def load_ncu_traffic(version):
-    """profiles/r2_traffic.csv: first line '# qk_version=<...>,size=256', then kernel,dram_read_gb,dram_write_gb."""
+    """profiles/r2_traffic.csv: first line '# qk_version=<...>;size=256', then kernel,dram_read_gb,dram_write_gb."""
     try:
         lines = open(os.path.join(ROOT, "profiles", "r2_traffic.csv")).read().splitlines()
-        meta = dict(kv.split("=", 1) for kv in lines[0].lstrip("# ").split(","))
+        meta = dict(kv.split("=", 1) for kv in lines[0].lstrip("# ").split(";"))
         if meta.get("qk_version") != version or int(meta.get("size", 0)) != 256:
             return
         for ln in lines[2:]:

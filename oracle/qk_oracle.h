@@ -21,10 +21,14 @@
  *        top-hat causality/positivity, conservation, split-diffusion factor
  *   orc_exchange_cell                       : eq 57 relaxation to 1e-5,
  *        bisection solution of the backward-Euler quartic, F_r decay closed form
+ *   default radiation flux (plain HLL, eps = 1)     : the radiation pressure tube, "better than 0.2 per cent"
+ *        (PAPER.md:484-494), which the opt-in optical-depth correction (ORC_FLAG_TAU_CORR, reading R6) misses
+ *   kappa(rho, T), eq 33 with d kappa_P/dT           : bisection of the backward-Euler scalar equation, Newton
+ *        iteration counts against the Jacobian without the term, kappa_F at the updated temperature
  *   PARITY UNPINNED (oracle<->GPU agreement only): the shock-flattening
- *        constants (PAPER.md:166 prints no formula), the wavespeed floor 0.1 c_hat,
- *        the form of the optical-depth correction and of its causality guard
- *        (PAPER.md:180-182 print no formula).
+ *        constants (PAPER.md:166 prints no formula), the VALUE 0.1 of the wavespeed floor (its reach is pinned:
+ *        it binds only for |f| > 0.99 grazing the face), the form of the opt-in optical-depth correction and of
+ *        its causality guard (PAPER.md:180-182 print no formula), the Minerbo polynomial (literature form).
  */
 #ifndef QK_ORACLE_H
 #define QK_ORACLE_H

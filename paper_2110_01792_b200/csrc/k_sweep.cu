@@ -36,7 +36,7 @@ struct HydroPhT {
     // select-only PPM limiter (same values): measured faster in the x sweep, slower in the marching sweeps
     static constexpr int BL_X = 1, BL_MARCH = 0;
     static constexpr bool CARRY = true;    // marching sweeps carry the raw interface value (measured: -1.5 %)
-    static constexpr int X_MINB = 5, Y_MINB = 4, Z_MINB = 3;
+    static constexpr int X_MINB = 5, Y_MINB = 4, Z_MINB = 3;     // z at 4 CTAs/SM (128 registers) spills: 0.81 -> 1.10 ms
     const double *w[5];        // rho, vx, vy, vz, P (ghost cells included)
     const double *chi;         // flattening coefficient of the cells -1..n
     double gamma;
@@ -253,13 +253,29 @@ int launch_chi(const Geom &g, double gamma, CHydro5 W, double *cx, double *cy, d
     return n;
 }
 
-// marching chunk: 32 cells, shorter for small boxes so that ~8 waves of warps stay available on 148 SMs x 16 warps
-static int sweep_len(int n_m, long long columns)
+// Marching chunk length.  A chunk of `len` cells costs len + ~3 cells of work (window prologue, two extra
+// reconstructions), so long chunks are cheaper per cell; but the launch must still fill the GPU with whole waves of
+// CTAs: with `ctas_per_sm` resident CTAs a grid of 9.2 waves runs for 10.  Among the lengths 16..64 take the one with
+// the least (work per cell) x (rounded-up waves / waves); boxes too small for ~8 waves of warps use short chunks.
+static int sweep_len(int n_m, int ctas_xy, int ctas_per_sm)
 {
-    int len = 32;
-    while (len > 8 && columns / 32 * ((n_m + len - 1) / len) < 148LL * 16 * 8) len /= 2;
-    if (len > n_m) len = n_m;
-    return len < 1 ? 1 : len;
+    const double per_wave = 148.0 * ctas_per_sm;
+    if ((double)ctas_xy * ((n_m + 31) / 32) < 2.0 * per_wave) {      // small box: more, shorter chunks
+        int len = 32;
+        while (len > 8 && (double)ctas_xy * ((n_m + len - 1) / len) < 2.0 * per_wave) len /= 2;
+        return len > n_m ? (n_m < 1 ? 1 : n_m) : len;
+    }
+    int best = 32;
+    double best_cost = 1e30;
+    for (int len = 16; len <= 64 && len <= n_m; ++len) {
+        const int chunks = (n_m + len - 1) / len;
+        const double waves = (double)ctas_xy * chunks / per_wave;
+        const double waves_up = (double)(long long)(waves + 0.999999);
+        // the last chunk of a column may be short: the longest chunk sets a CTA's time
+        const double cost = (1.0 + 3.0 / len) * (waves_up / waves) * ((double)chunks * len / n_m);
+        if (cost < best_cost - 1e-12) { best_cost = cost; best = len; }
+    }
+    return best;
 }
 
 template <class PH>
@@ -277,13 +293,13 @@ static int launch_sweeps(const PH &ph, const Geom &g, double dtdx, int stage, Fi
     }
     const int bx = (g.nx + SW_NT - 1) / SW_NT;
     if ((which & 2) && k1 > k0) {        // y sweep of the planes [k0, k1)
-        const int len = sweep_len(g.ny, (long long)g.nx * g.nz);
+        const int len = sweep_len(g.ny, bx * (k1 - k0), PH::Y_MINB);
         dim3 grid(bx, k1 - k0, (g.ny + len - 1) / len);
         sweep_march_kernel<PH, 1><<<grid, SW_NT, 0, st>>>(ph, g, len, k0, D, rk, U, U0, out, pout, ctr, cache);
         ++n;
     }
     if (which & 4) {                     // z sweep: always the whole box
-        const int len = sweep_len(g.nz, (long long)g.nx * g.ny);
+        const int len = sweep_len(g.nz, bx * g.ny, PH::Z_MINB);
         dim3 grid(bx, g.ny, (g.nz + len - 1) / len);
         sweep_march_kernel<PH, 2><<<grid, SW_NT, 0, st>>>(ph, g, len, 0, D, rk, U, U0, out, pout, ctr, cache);
         ++n;
