@@ -199,6 +199,7 @@ class Context:
     # ---- one method per C entry point -----------------------------------------------------------
     def qk_set_stream(self, cuda_stream):
         _check(self.L.qk_set_stream(self.h, C.c_void_p(cuda_stream)), "qk_set_stream")
+        self.stream_ptr = int(cuda_stream)
 
     def qk_set_constants(self, a_rad, kB_over_mu_mH):
         _check(self.L.qk_set_constants(self.h, a_rad, kB_over_mu_mH), "qk_set_constants")

@@ -47,6 +47,13 @@ class TorchTransport:
         self.dist = dist
         self.group = group
 
+    def device_stream(self):
+        """raw handle of the stream NCCL orders its point-to-point operations against (None on CPU backends)"""
+        import torch
+        if self.dist.get_backend(self.group) != "nccl":
+            return None
+        return int(torch.cuda.current_stream().cuda_stream)
+
     def exchange(self, lo, hi, send_lo, send_hi, recv_lo, recv_hi):
         dist = self.dist
         ops = []
@@ -95,6 +102,12 @@ class SlabExchange:
         # called by the library before every ghost fill; exceptions cannot cross the C frame: a non-zero return
         # makes the step call fail and later step calls return QK_EINVAL until the exchange is attached again
         try:
+            # the point-to-point operations order against torch's current stream, pack / unpack against the context's
+            # stream: they must be the same one
+            sp = getattr(self.ctx, "stream_ptr", None)
+            ts = self.transport.device_stream() if hasattr(self.transport, "device_stream") else None
+            if sp is not None and ts is not None:
+                assert ts == sp, "halo exchange: torch's current stream is not the context's stream"
             send_lo, send_hi, recv_lo, recv_hi = self._bufs(nfields)
             if self.lo is not None:
                 self.ctx.qk_halo_pack(FACE_ZLO, send_lo)
