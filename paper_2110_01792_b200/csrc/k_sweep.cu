@@ -36,7 +36,10 @@ struct HydroPhT {
     // select-only PPM limiter (same values): measured faster in the x sweep, slower in the marching sweeps
     static constexpr int BL_X = 1, BL_MARCH = 0;
     static constexpr bool CARRY = true;    // marching sweeps carry the raw interface value (measured: -1.5 %)
-    static constexpr int X_MINB = 5, Y_MINB = 4, Z_MINB = 3;     // z at 4 CTAs/SM (128 registers) spills: 0.81 -> 1.10 ms
+    // CTAs per SM.  z runs at 4 (126 registers, no spill) only because its update inputs are staged by cp.async and
+    // never sit in registers during the Riemann solve: 0.81 -> 0.77 ms; with register loads 4 CTAs spill (1.10 ms).
+    // y at 5 (96 registers) spills: 0.62 -> 0.78 ms.  x at 6 (78 registers): no gain, it is pipe-bound.
+    static constexpr int X_MINB = 5, Y_MINB = 4, Z_MINB = 4;
     const double *w[5];        // rho, vx, vy, vz, P (ghost cells included)
     const double *chi;         // flattening coefficient of the cells -1..n
     double gamma;
@@ -129,7 +132,7 @@ struct RadPhT {
     static constexpr bool COUNTS = true;
     static constexpr int BL_X = 1, BL_MARCH = 1;
     static constexpr bool CARRY = false;   // measured slower with the select-only limiter (+1.5 %)
-    static constexpr int X_MINB = 5, Y_MINB = 4, Z_MINB = 3;
+    static constexpr int X_MINB = 5, Y_MINB = 4, Z_MINB = 4;
     const double *s[4];        // E_r, fx, fy, fz
     const double *rho, *kR;
     double c, c_hat, dx;

@@ -11,7 +11,9 @@
 //   sweep_march_kernel : one thread per (x, other) column marching along y or z over a chunk of cells; the
 //                        five-cell window of the column lives in a thread-private shared-memory ring (no barrier
 //                        anywhere), the high face state, the low-face flux and the raw eq 22 interface value of
-//                        the previous cell stay in registers.  y: D += dF_y.  z: RK stage update
+//                        the previous cell stay in registers; the own-cell inputs of the update are copied global ->
+//                        shared by cp.async at the top of a step and read at its end (they never occupy registers
+//                        during the Riemann solve: that is what lets the z sweep run at 4 CTAs per SM).  y: D += dF_y.  z: RK stage update
 //                        with (dF_x + dF_y) + dF_z (the paper's sum order) and, after the last hydro
 //                        stage, the CFL signal speed of the new state (eq 21).
 //
@@ -158,6 +160,8 @@ __global__ void __launch_bounds__(SW_NT, DIR == 2 ? PH::Z_MINB : PH::Y_MINB) swe
     const double dtdx = (DIR == 2 && rk.dtdx_dev) ? __ldg(rk.dtdx_dev) : rk.dtdx;
     typename PH::Tail tail;                             // per-thread reduction state of the z epilogue
     __shared__ double ring[5 * SW_NR * SW_NT];          // [slot][var][thread], thread-private columns
+    // own-cell inputs of the update (D; for z also U and U^n), staged global -> shared by cp.async: [array][var][thread]
+    __shared__ double own[(DIR == 2 ? 3 : 1) * PH::NV * SW_NT];   // z: D, U, U^n of the cell being updated, staged by cp.async
     const int tid = threadIdx.x;
     const int i = blockIdx.x * SW_NT + tid;
     const bool active = i < g.nx;
@@ -207,15 +211,17 @@ __global__ void __launch_bounds__(SW_NT, DIR == 2 ? PH::Z_MINB : PH::Y_MINB) swe
         }
         const int cidx = base + m * s;
         // own-cell inputs of the update, consumed at the end of the step
-        double din[NV], u[NV], u0[NV];
         if (m >= m0) {
+            {     // global -> shared without passing through registers: they land while the Riemann solve runs
 #pragma unroll
-            for (int v = 0; v < NV; ++v) {
-                din[v] = D.f[v][cidx];
-                if (DIR == 2) {
-                    u[v] = U.f[v][cidx];
-                    u0[v] = rk.stage == 1 ? U0.f[v][cidx] : 0.0;
+                for (int v = 0; v < NV; ++v) {
+                    cp_async8(&own[(0 * NV + v) * SW_NT + tid], D.f[v] + cidx);
+                    if (DIR == 2) {
+                        cp_async8(&own[(1 * NV + v) * SW_NT + tid], U.f[v] + cidx);
+                        if (rk.stage == 1) cp_async8(&own[(2 * NV + v) * SW_NT + tid], U0.f[v] + cidx);
+                    }
                 }
+                cp_async_commit();
             }
         }
         // limited face states of cell m+1
@@ -233,16 +239,18 @@ __global__ void __launch_bounds__(SW_NT, DIR == 2 ? PH::Z_MINB : PH::Y_MINB) swe
             const int mm = m + 1;
             if (PH::COUNTS && active && ((mm >= m0 && mm < m1) || mm == n_m)) nguard += gd;
         }
+        if (m >= m0) cp_async_wait<0>();
         if (m >= m0 && active) {
             double fresh[NV];
 #pragma unroll
             for (int v = 0; v < NV; ++v) {
-                const double div = din[v] + (Fhi[v] - Flo[v]);              // dF_x + dF_y, then (dF_x + dF_y) + dF_z
+                const double dv = own[(0 * NV + v) * SW_NT + tid];
+                const double div = dv + (Fhi[v] - Flo[v]);                  // dF_x + dF_y, then (dF_x + dF_y) + dF_z
                 if (DIR == 1) {
                     D.f[v][cidx] = div;
                 } else {
-                    const double us = u[v] - dtdx * div;
-                    fresh[v] = rk.stage == 0 ? us : 0.5 * u0[v] + 0.5 * us;
+                    const double us = own[(1 * NV + v) * SW_NT + tid] - dtdx * div;
+                    fresh[v] = rk.stage == 0 ? us : 0.5 * own[(2 * NV + v) * SW_NT + tid] + 0.5 * us;
                     out.f[v][cidx] = fresh[v];
                 }
             }
