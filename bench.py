@@ -53,6 +53,7 @@ SCHEME_FLAGS = 0            # --plm / --eddington: scheme variants (PAPER.md:164
 # profiles/r2_kernels.md, valid for the library version named in the csv; bench.py checks qk_version() against it
 # and reports null otherwise (the field is labelled "traffic_source": a static capture, not a live counter)
 NCU_TRAFFIC_GB_256 = {}     # kernel class -> GB per launch, read from profiles/r2_traffic.csv
+HBM_GBS = 6650.0            # set from MEASURED_PEAKS.json in run_ours
 
 
 def load_ncu_traffic(version):
@@ -393,6 +394,8 @@ def roofline_alu(kernel_ms, names, ops_per_cell_per_launch, cells, peak_ops, pea
             "traffic": None if traffic is None else traffic * 1e9,
             "traffic_source": "profiles/r2_traffic.csv (ncu --set full capture of this library version; static, not live)"
                               if traffic is not None else None,
+            # the same launch against the HBM roof, on the bytes it really moves (informative: `frac` is the headline)
+            "frac_hbm_on_traffic": None if traffic is None else traffic * 1e9 / (mean_ms * 1e-3) / (HBM_GBS * 1e9),
             "launch_ms": mean_ms, "launches": cnt, "peak_source": peak_note,
             "ops_per_cell_per_launch": ops_per_cell_per_launch}
 
@@ -445,7 +448,8 @@ def run_ours(args):
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
     except Exception:
         pass
-    hbm = float(peaks.get("hbm_gbs", 6650.0))
+    global HBM_GBS
+    hbm = HBM_GBS = float(peaks.get("hbm_gbs", 6650.0))
     hbm_note = "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
     peak_note = "qk_fp64_probe: measured DMUL+DADD lane-ops/s on this GPU (DFMA probe: %.2f T/s)" % (peak_fma / 1e12)
     single = world == 1
