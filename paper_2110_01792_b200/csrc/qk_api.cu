@@ -795,8 +795,12 @@ int qk_set_halo_peers(qk_ctx *c, const qk_halo_handle *lo, const qk_halo_handle 
             cudaIpcMemHandle_t ih;
             memcpy(&ih, h->ipc, sizeof(ih));
             void *mapped = nullptr;
-            if (cudaIpcOpenMemHandle(&mapped, ih, cudaIpcMemLazyEnablePeerAccess) != cudaSuccess) { cudaGetLastError(); return QK_ECUDA; }
-            c->peer[p].ipc_ptr = mapped;
+            if (p == 1 && lo && c->peer[0].ipc_ptr && lo->pid == h->pid && lo->base == h->base) {
+                mapped = c->peer[0].ipc_ptr;        // two ranks, periodic: both neighbours are the one peer -- one mapping, owned by peer[0]
+            } else {
+                if (cudaIpcOpenMemHandle(&mapped, ih, cudaIpcMemLazyEnablePeerAccess) != cudaSuccess) { cudaGetLastError(); return QK_ECUDA; }
+                c->peer[p].ipc_ptr = mapped;
+            }
             base = (char *)mapped + h->offset;
         }
         qk_ctx::Peer &pr = c->peer[p];
