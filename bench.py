@@ -367,7 +367,7 @@ def run_workload(torch, B, I, kind, params, fields, steps, warmup, rank, world, 
             out["halo"] = {"exchange": how, "exchanges": getattr(ex, "calls", None),
                            "bytes_sent_per_rank": getattr(ex, "bytes_sent", None)}
             ex.detach()
-    if e2e and ex is None and kind != "rad":
+    if e2e and kind != "rad":
         e2e_steps = max(3, min(steps, 12))
         nsub = max(1, out["info"]["nsub"])
         ms_e = allmax(time_e2e(torch, B, I, params, fields, kind, nf, e2e_steps, barrier, nsub))
@@ -375,7 +375,8 @@ def run_workload(torch, B, I, kind, params, fields, steps, warmup, rank, world, 
                       "h2d_bytes_per_step": nf * cells * 8, "d2h_bytes_per_step": nf * cells * 8,
                       "ms_per_step": ms_e / e2e_steps, "steps": e2e_steps,
                       "how": "qk_set_state_all + %s + qk_get_state_all per step, pinned host buffers, three boxes in flight"
-                             % ("qk_hydro_step_cfl" if kind == "hydro" else "qk_rhd_step_cfl(%d)" % nsub)}
+                             % ("qk_hydro_step_cfl" if kind == "hydro" else "qk_rhd_step_cfl(%d)" % nsub)
+                             + ("" if world == 1 else "; every rank streams periodic boxes of its own (no halo exchange on this leg)")}
     return out
 
 
@@ -418,11 +419,16 @@ def run_ours(args):
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.backend == "gloo":          # functional check of the decomposed path on a box with fewer GPUs than ranks
+        local %= torch.cuda.device_count()
     torch.cuda.set_device(local)
     dist = None
     if world > 1:
         import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if args.backend == "gloo":
+            dist.init_process_group("gloo")
+        else:
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     def barrier():
         if dist is not None:
@@ -647,6 +653,9 @@ def main():
     ap.add_argument("--no-512", action="store_true", help="leave out the 512^3 sub-record (its inputs take ~2 min to generate)")
     ap.add_argument("--quick", action="store_true", help="only the hydro and RHD workloads at --size (no sub-records)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"],
+                    help="torch.distributed backend for N > 1; gloo lets ranks share a GPU (rank r uses cuda:r mod #GPUs): "
+                         "a functional check of the decomposed path only -- ranks time-slice, the numbers mean nothing")
     args = ap.parse_args()
     global SCHEME_FLAGS, HYDRO_WORKLOAD
     HYDRO_WORKLOAD = args.workload

@@ -44,3 +44,27 @@ def test_own_arm_line_has_the_contract_keys():
     assert d["cpu_baseline"]["one_core"]["cores"] == 1 and d["cpu_baseline"]["cores"] >= 1
     if d["clocks"] is not None:
         assert {"sm_mhz", "sm_max_mhz", "reasons"} <= set(d["clocks"])
+
+
+@pytest.mark.gpu
+def test_own_arm_two_ranks_decomposed_box_runs_under_torchrun():
+    """`bench.py --gpus 2` as the driver launches it, except for `--backend gloo` so that both ranks can share the one
+    GPU of this box: the decomposed path (peer-mapped exchange across processes, global dt, max over ranks) runs, rank 0
+    alone prints the line, and the line says how the halos travelled.  The timings of two time-slicing ranks mean
+    nothing and are not looked at."""
+    import socket
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr",
+           "127.0.0.1", "--master-port", str(port), os.path.join(ROOT, "bench.py"), "--gpus", "2", "--size", "32",
+           "--steps", "3", "--warmup", "3", "--rhd-steps", "2", "--no-cpu-baseline", "--backend", "gloo"]
+    r = subprocess.run(cmd, capture_output=True, text=True, cwd=ROOT, timeout=600,
+                       env=dict(os.environ, OMP_NUM_THREADS="1", GLOO_SOCKET_IFNAME="lo"))
+    assert r.returncode == 0, (r.stdout[-1500:], r.stderr[-3000:])
+    lines = [l for l in r.stdout.splitlines() if l.strip().startswith("{")]
+    assert len(lines) == 1, lines
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["scaling"] == "weak" and d["value"] > 0 and d["gpu_launches"] > 0
+    assert "z-slab decomposition" in d["config"]["parallelism"] and "peer-mapped" in d["halo"]["exchange"]
+    assert d["e2e"]["value"] > 0 and d["rhd"]["value"] > 0
