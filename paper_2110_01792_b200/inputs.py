@@ -169,6 +169,26 @@ def sedov(n=256):
     return params, _fill_missing(_hydro_fields(np.ones(shape), z, z.copy(), z.copy(), P, gamma), shape)
 
 
+def su_olson(n=1500):
+    """The paper's Su-Olson problem (eq 56) with every printed parameter: a_r = c = 1, no reduced
+    speed of light, kappa_P = kappa_R = 1, rho = 1, gas at rest (v/c terms dropped), source Q a_r T_H^4 = 1 in
+    0 <= x < x_0 = 0.5 while t < t_0 = 10, initial E_g = E_r = 1e-10, reflecting walls on [0, 30], N_x = 1500, CFL 0.4,
+    heat capacity C_v = alpha T^3 with alpha = 4 a_r / epsilon, epsilon = 1 (eq 55).  One row of cells in y and z.
+    Returns (params, fields, extra): extra holds what the generic setters do not (source rate, EOS, end time)."""
+    shape = (1, 1, n)
+    L, x0, t0 = 30.0, 0.5, 10.0
+    dx = L / n
+    x = _centres(n, 0.0, L)
+    e0 = 1e-10
+    fields = {"rho": np.ones(shape), "E": np.full(shape, e0), "Er": np.full(shape, e0),
+              "kappaP": np.ones(shape), "kappaR": np.ones(shape)}
+    src = np.where(x < x0, 1.0 / (2.0 * x0), 0.0).reshape(shape)
+    params = dict(nx=n, ny=1, nz=1, dx=dx, gamma=5.0 / 3.0, c_hat=1.0, c=1.0, bc=BC_REFLECTING, cfl=0.4,
+                  a_rad=1.0, kB_mu=1.0, flags=FLAG_STATIC_MATTER, name="su_olson")
+    extra = dict(src=np.ascontiguousarray(src), eos_alpha=4.0, t_end=t0, x0=x0, dt=0.4 * dx / 1.0, e_init=e0, length=L)
+    return params, _fill_missing(fields, shape), extra
+
+
 def ragged_hydro(shape=(19, 22, 37), seed=7, bc=BC_PERIODIC, mach=1.5):
     """Small non-cubic, non-multiple-of-tile box with shocks: several tiles and a ragged tail."""
     p, f = config2(seed=seed, mach=mach, kmax=3, shape=shape)

@@ -1238,3 +1238,33 @@ def test_halo_callback_failure_aborts_the_step():
             ctx.qk_hydro_step_cfl()
         ctx.qk_set_halo_exchange(0, None)
         ctx.qk_hydro_step(1e-4)
+
+
+# ------------------------------------------------------------------------------------------------
+# The paper's Su-Olson problem on the CUDA path
+# ------------------------------------------------------------------------------------------------
+def test_su_olson_problem_with_the_papers_parameters():
+    """Every printed parameter (source of eq 56, reflecting walls on [0, 30], N_x = 1500, CFL 0.4, C_v = alpha T^3, gas
+    at rest, c_hat = c), run to t_0 = 10: the energy budget sum (E_g + E_r) dx = 5 + initial to round-off, causality,
+    the gas lagging the radiation, a monotone wave (tests/test_oracle_su_olson.py states why these and not the
+    Su & Olson tables); and the state after 250 steps equal to the oracle's bit for bit."""
+    from test_oracle_su_olson import check_su_olson, su_olson_oracle
+    params, fields, extra = I.su_olson(1500)
+    _, _, osteps, oref, oinfo = su_olson_oracle(1500, 250)
+    with P.make_gpu(params, fields) as ctx:
+        ctx.qk_set_eos(B.QK_EOS_ALPHA_T3, extra["eos_alpha"])
+        ctx.qk_set_state(B.FIELDS.index("src"), extra["src"])
+        nsteps = int(round(extra["t_end"] / extra["dt"]))
+        assert nsteps == 1250
+        for s in range(1, nsteps + 1):
+            ctx.qk_rad_step(extra["dt"])
+            if s == osteps:
+                got = {k: ctx.qk_get_state(B.FIELDS.index(k)).ravel() for k in ("E", "Er", "Fx", "mx")}
+                P.assert_bitwise(oref, got, ["E", "Er", "Fx", "mx"], "Su-Olson after %d steps" % s)
+                assert ctx.qk_last_info()["newton_total_iters"] == oinfo["newton_total_iters"]
+        out = {k: ctx.qk_get_state(B.FIELDS.index(k)).ravel() for k in ("E", "Er", "Fx", "mx")}
+        info = ctx.qk_last_info()
+    assert info["status"] == 0
+    budget, Er = check_su_olson(params, extra, nsteps, out, info)
+    assert abs(budget - 5.0) < 1e-8                                  # 5 + 30 * 2e-10
+    assert Er.argmax() == 0 and Er[int(9.0 / params["dx"])] < 1e-2 * Er[0]
