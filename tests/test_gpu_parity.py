@@ -1268,3 +1268,48 @@ def test_su_olson_problem_with_the_papers_parameters():
     budget, Er = check_su_olson(params, extra, nsteps, out, info)
     assert abs(budget - 5.0) < 1e-8                                  # 5 + 30 * 2e-10
     assert Er.argmax() == 0 and Er[int(9.0 / params["dx"])] < 1e-2 * Er[0]
+
+
+def test_gpu_slow_moving_shock_speed():
+    """PAPER.md:357-366 on the CUDA path: the shock of the Jin & Liu states moves at the printed 0.1096, ~250 steps per
+    cell at CFL 0.2, per-cent post-shock oscillation; the state at t = 1 equals the oracle's bit for bit (about 2700
+    steps with the timestep taken from each side's own eq 21 -- so the timesteps agree bit for bit as well)."""
+    from test_oracle_hydro import SLOW_SHOCK, shock_position, slow_shock_ic
+    N, gamma = 100, SLOW_SHOCK["gamma"]
+    x = (np.arange(N) + 0.5) / N
+    rho, vx, Pr = slow_shock_ic(x)
+    U0 = [rho, rho * vx, 0 * x, 0 * x, Pr / (gamma - 1) + 0.5 * rho * vx * vx]
+    g = O.Grid(N, 1, 1, 1.0 / N, gamma, bc=O.BC_OUTFLOW)
+    g.set_params(cfl=0.2)
+    level = 0.5 * (SLOW_SHOCK["L"][0] + SLOW_SHOCK["R"][0])
+    with B.Context(N, 1, 1, 1.0 / N, gamma, 0.0, 0.0, B.QK_BC_OUTFLOW) as ctx:
+        ctx.qk_set_params(cfl=0.2, flags=0)
+        for k in range(5):
+            ctx.qk_set_state(k, U0[k].reshape(1, 1, N))
+            g.set_state(k, U0[k].reshape(1, 1, N))
+        pos, t, steps = [], 0.0, 0
+        threads = O.get_threads()
+        O.set_threads(1)
+        try:
+            for t_end in (1.0, 2.0):
+                while t < t_end * (1 - 1e-14):
+                    dt = min(ctx.qk_cfl_dt(), t_end - t)
+                    if t_end == 1.0:
+                        assert dt == min(g.cfl_dt(), t_end - t)
+                        assert g.hydro_step(dt) == 0
+                    ctx.qk_hydro_step(dt)
+                    t += dt
+                    steps += 1
+                got = [ctx.qk_get_state(k).ravel() for k in range(5)]
+                if t_end == 1.0:
+                    for k in range(5):
+                        assert np.array_equal(got[k], g.get_state(k).ravel()), k
+                pos.append(shock_position(x, got[0], level))
+        finally:
+            O.set_threads(threads)
+            g.close()
+        assert ctx.qk_last_info()["status"] == 0
+    assert abs((pos[1] - pos[0]) - SLOW_SHOCK["speed"]) < 0.5 / N, pos
+    assert 200 < steps / (N * (pos[1] - 0.5)) < 300
+    post = got[0][x < pos[1] - 0.05]
+    assert np.abs(post / SLOW_SHOCK["L"][0] - 1.0).max() < 0.02 and np.abs(got[0][x > pos[1] + 0.03] - 1.0).max() < 1e-6

@@ -180,7 +180,63 @@ def test_strong_shock_tube_error_scale():
     Uex = [r, r * u, p / (g - 1) + 0.5 * r * u * u]
     num = np.sqrt(np.mean([np.abs(U[k] - Uex[n]).mean() ** 2 for n, k in enumerate((0, 1, 4))]))
     den = np.sqrt(np.mean([np.abs(Uex[n]).mean() ** 2 for n in range(3)]))
-    assert 0.5e-3 < num / den < 2.5e-3, num / den
+    # paper: 1.12e-3 (gamma = 1.4 gives 1.19e-3 here, gamma = 5/3 1.31e-3); within 20 % of the printed value -- without
+    # flattening the paper reports "unacceptably large post-shock oscillations", so this holds the H6 constants to scale
+    assert 0.9e-3 < num / den < 1.35e-3, num / den
+
+
+SLOW_SHOCK = dict(gamma=1.4, L=(3.86, -3.1266, 27.0913), R=(1.0, -3.44, 8.4168), speed=0.1096)
+
+
+def slow_shock_ic(x):
+    g = SLOW_SHOCK["gamma"]
+    (rl, ml, el), (rr, mr, er) = SLOW_SHOCK["L"], SLOW_SHOCK["R"]
+    pl, pr = (g - 1) * (el - 0.5 * ml * ml / rl), (g - 1) * (er - 0.5 * mr * mr / rr)
+    left = x < 0.5
+    return np.where(left, rl, rr), np.where(left, ml / rl, mr / rr), np.where(left, pl, pr)
+
+
+def shock_position(x, rho, level):
+    """where rho falls through `level`, linearly interpolated between cell centres (last crossing from the left)"""
+    j = np.nonzero(rho > level)[0][-1]
+    return x[j] + (rho[j] - level) / (rho[j] - rho[j + 1]) * (x[j + 1] - x[j])
+
+
+def test_slow_moving_shock_speed():
+    """PAPER.md:357-366 (Jin & Liu parameters, gamma = 1.4, CFL 0.2): 'the shock jump moving to the right with a
+    velocity v_shock = 0.1096', ~250 steps per cell.  The density jump's midpoint travels at that speed (between t = 1
+    and t = 2, after the start-up waves of the rounded printed states have left), the post-shock oscillation the
+    paper describes stays at the per-cent level with flattening, and nothing overshoots on the pre-shock side."""
+    N = 100
+    gamma = SLOW_SHOCK["gamma"]
+    g = O.Grid(N, 1, 1, 1.0 / N, gamma, bc=O.BC_OUTFLOW)
+    g.set_params(cfl=0.2)
+    x = (np.arange(N) + 0.5) / N
+    rho, vx, P = slow_shock_ic(x)
+    for k, a in enumerate([rho, rho * vx, 0 * x, 0 * x, P / (gamma - 1) + 0.5 * rho * vx * vx]):
+        g.set_state(k, a.reshape(1, 1, N))
+    threads = O.get_threads()
+    O.set_threads(1)                   # one row of cells, ~5000 steps: the thread team would cost more than the loops
+    pos, t, steps = [], 0.0, 0
+    try:
+        for t_end in (1.0, 2.0):
+            while t < t_end * (1 - 1e-14):
+                dt = min(g.cfl_dt(), t_end - t)
+                assert g.hydro_step(dt) == 0
+                t += dt
+                steps += 1
+            U = [g.get_state(0).ravel()]
+            pos.append(shock_position(x, U[0], 0.5 * (SLOW_SHOCK["L"][0] + SLOW_SHOCK["R"][0])))
+    finally:
+        O.set_threads(threads)
+        g.close()
+    assert 200 < steps / (N * (pos[1] - 0.5)) < 300          # "~250 timesteps to move across a single cell"
+    speed = pos[1] - pos[0]
+    assert abs(speed - SLOW_SHOCK["speed"]) < 0.5 / N, (pos, speed)
+    post = U[0][x < pos[1] - 0.05]
+    assert np.abs(post / SLOW_SHOCK["L"][0] - 1.0).max() < 0.02
+    pre = U[0][x > pos[1] + 0.03]
+    assert np.abs(pre - 1.0).max() < 1e-6
 
 
 def test_advected_wave_second_order():
