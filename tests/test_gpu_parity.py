@@ -1366,3 +1366,28 @@ def test_gpu_radiation_driven_wind_follows_eq61():
     err = np.abs(M / s["M"] - 1.0)
     assert err.max() < 3e-3, err.max()
     assert np.abs(U[6] / s["F0"] - 1.0).max() < 1e-5 and np.abs(U[0] * M / (3.897212e-19 * 1.1) - 1.0).max() < 5e-3      # rho M = rho_0 M_0
+
+
+# ------------------------------------------------------------------------------------------------
+# the Marshak wave, every printed parameter (reading B3 for the inflow face)
+# ------------------------------------------------------------------------------------------------
+def test_gpu_marshak_wave():
+    """400 cells on 20 mean free paths, hohlraum at 3.481334e6 K behind the left face, C_v = alpha T^3, c_hat = c, 500
+    steps at CFL 0.4 to tau = 10: the CUDA path's wave equals the oracle's bit for bit (Newton iteration counts included)
+    and passes the same comparison with the independent diffusion solution (tests/test_oracle_marshak.py)."""
+    import test_oracle_marshak as M
+    s, ref_out, ref_info = M.run_oracle("bath")
+    with B.Context(s["N"], 1, 1, s["dx"], 5.0 / 3.0, M.C_LIGHT, M.C_LIGHT) as ctx:
+        ctx.qk_set_constants(M.A_RAD, 1.0)
+        ctx.qk_set_params(cfl=0.4, flags=B.QK_FLAG_STATIC_MATTER)
+        ctx.qk_set_eos(B.QK_EOS_ALPHA_T3, s["alpha"])
+        ctx.qk_set_face_boundaries([B.QK_BC_FIXED, B.QK_BC_OUTFLOW, 0, 0, 0, 0])
+        for f, a in s["raw"].items():
+            ctx.qk_set_raw(f, a)
+        for _ in range(s["nsteps"]):
+            ctx.qk_rad_step(s["dt"])
+        out = {k: ctx.qk_get_state(f).ravel() for k, f in (("E", 4), ("Er", 5), ("Fx", 6))}
+        info = ctx.qk_last_info()
+    assert info["status"] == 0 and info["newton_total_iters"] == ref_info["newton_total_iters"]
+    P.assert_bitwise(ref_out, out, ["E", "Er", "Fx"], "Marshak wave after %d steps" % s["nsteps"])
+    M.check_marshak(s, out, M.diffusion_reference())
