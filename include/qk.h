@@ -262,6 +262,13 @@ long long qk_launch_count(const qk_ctx *ctx);
  * bracketed groups per class into ms[]/count[] (arrays of qk_kernel_class_count() entries) and
  * clears the record. */
 int qk_set_profiling(qk_ctx *ctx, int on);
+
+/* Which implementation of the flattening coefficient (H6) a hydro stage launches:
+ * 0 = by box size (default), 1 = two pointwise passes through three chi~ arrays (faster while those stay in
+ * L2, boxes up to ~160^3), 2 = one z-marching pass without chi~ arrays (half the HBM bytes; faster beyond).
+ * Both give the same bits; the switch exists so that tests and measurements can run either on any box.
+ * QK_EINVAL for another value. */
+int qk_set_flatten_path(qk_ctx *ctx, int path);
 int qk_kernel_class_count(void);
 const char *qk_kernel_class_name(int cls);
 int qk_kernel_times(qk_ctx *ctx, double *ms, long long *count);

@@ -26,7 +26,7 @@ EXPORTS = [
     "qk_init", "qk_free", "qk_state_bytes", "qk_bind_storage", "qk_set_stream", "qk_set_constants",
     "qk_set_params", "qk_set_state", "qk_get_state", "qk_set_raw", "qk_get_raw", "qk_fill_boundary",
     "qk_cfl_dt", "qk_hydro_step", "qk_rad_transport", "qk_exchange", "qk_rad_step", "qk_rhd_step",
-    "qk_nsub_for", "qk_last_info", "qk_launch_count", "qk_set_profiling",
+    "qk_nsub_for", "qk_last_info", "qk_launch_count", "qk_set_profiling", "qk_set_flatten_path",
     "qk_kernel_class_count", "qk_kernel_class_name", "qk_kernel_times", "qk_version", "qk_fp64_probe",
     "qk_selftest_divsqrt", "qk_set_eos", "qk_set_opacity_law", "qk_set_opacity_law_T", "qk_set_face_boundaries",
     "qk_hydro_step_cfl", "qk_rhd_step_cfl", "qk_last_dt", "qk_set_halo_exchange", "qk_halo_doubles", "qk_halo_pack",
@@ -100,6 +100,7 @@ def lib():
         "qk_last_info": (i, [p, C.POINTER(qk_info)]),
         "qk_launch_count": (ll, [p]),
         "qk_set_profiling": (i, [p, i]),
+        "qk_set_flatten_path": (i, [p, i]),
         "qk_kernel_class_count": (i, []),
         "qk_kernel_class_name": (C.c_char_p, [i]),
         "qk_kernel_times": (i, [p, C.POINTER(d), C.POINTER(ll)]),
@@ -348,6 +349,9 @@ class Context:
 
     def qk_set_profiling(self, on):
         _check(self.L.qk_set_profiling(self.h, int(on)), "qk_set_profiling")
+
+    def qk_set_flatten_path(self, path):
+        _check(self.L.qk_set_flatten_path(self.h, int(path)), "qk_set_flatten_path")
 
     def qk_kernel_times(self):
         n = self.L.qk_kernel_class_count()

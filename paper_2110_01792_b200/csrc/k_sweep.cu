@@ -301,13 +301,102 @@ __global__ void __launch_bounds__(128) chi_min2_kernel(Geom g, int k0, const dou
     else chi[c] = r.x;
 }
 
+// ---- flattening coefficient in ONE pass, no chi~ arrays ------------------------------------------------------
+// One thread per (i, j) column of [-1, nx] x [-1, ny] marching along z over a chunk of planes.  chi~_z of the three
+// planes k-1, k, k+1 comes from a register window of the column's own P and v_z (each evaluated once); chi~_x and
+// chi~_y of the three neighbours along x and y are evaluated in place from P and v_x / v_y of the cell's row and
+// of the rows j +- 1..3 -- those loads are L1 / L2 hits on lines the neighbouring lanes and warps fetch anyway.
+// No shared memory, no barrier (the rejected one-kernel variant of round 2, paid one barrier
+// per plane).  HBM traffic: P, v once and chi once, 44 B/cell measured instead of the two passes' 89.
+// The value is the two-pass result bit for bit: the same flatten_coeff_1d on the same operands, and the same
+// nesting of the minimum.
+// 32 x 4 tiles at 5 CTAs per SM (96 registers, no spill): 0.250 ms at 256^3; 32 x 8 at 3 (80 registers, 76 B of
+// spills) 0.275 ms, 32 x 2 at 10: 0.253 ms; grouping the loads by direction instead of issuing all 24 first: 0.35 ms.
+constexpr int CHI_TX = 32, CHI_TY = 4, CHI_MINB = 5;
+
+__global__ void __launch_bounds__(CHI_TX * CHI_TY, CHI_MINB) chi_march_kernel(Geom g, int m0, int m1, int len, double gamma,
+                                                                    const double *__restrict__ P, const double *__restrict__ vx,
+                                                                    const double *__restrict__ vy, const double *__restrict__ vz,
+                                                                    double *__restrict__ chi)
+{
+    const int i = (int)blockIdx.x * CHI_TX + (int)threadIdx.x - 1;
+    const int j = (int)blockIdx.y * CHI_TY + (int)threadIdx.y - 1;
+    if (i > g.nx || j > g.ny) return;
+    const int ka = m0 + (int)blockIdx.z * len, kb = min(ka + len, m1);
+    const int sy = g.sy, sz = g.sz;
+    int c = g.at(i, j, ka);
+    // z window of the column: P(k-1..k+2), v_z(k), v_z(k+1); chi~_z(k-1), chi~_z(k)
+    double pa, pb, pc, pd, wa, wb, czm, cz0;
+    {
+        const double q3 = __ldg(P + c - 3 * sz), q2 = __ldg(P + c - 2 * sz);
+        pa = __ldg(P + c - sz); pb = __ldg(P + c); pc = __ldg(P + c + sz); pd = __ldg(P + c + 2 * sz);
+        const double u2 = __ldg(vz + c - 2 * sz), u1 = __ldg(vz + c - sz);
+        wa = __ldg(vz + c); wb = __ldg(vz + c + sz);
+        czm = flatten_coeff_1d(gamma, q3, q2, pa, pb, pc, u2, wa);
+        cz0 = flatten_coeff_1d(gamma, q2, pa, pb, pc, pd, u1, wb);
+    }
+    for (int k = ka; k < kb; ++k, c += sz) {
+        // all 24 loads of the step are issued before the first evaluation: the kernel lives on memory-level parallelism
+        const double pe = __ldg(P + c + 3 * sz), wc = __ldg(vz + c + 2 * sz);
+        const double xm3 = __ldg(P + c - 3), xm2 = __ldg(P + c - 2), xm1 = __ldg(P + c - 1);
+        const double xp1 = __ldg(P + c + 1), xp2 = __ldg(P + c + 2), xp3 = __ldg(P + c + 3);
+        const double um2 = __ldg(vx + c - 2), um1 = __ldg(vx + c - 1), u0 = __ldg(vx + c), up1 = __ldg(vx + c + 1), up2 = __ldg(vx + c + 2);
+        const double ym3 = __ldg(P + c - 3 * sy), ym2 = __ldg(P + c - 2 * sy), ym1 = __ldg(P + c - sy);
+        const double yp1 = __ldg(P + c + sy), yp2 = __ldg(P + c + 2 * sy), yp3 = __ldg(P + c + 3 * sy);
+        const double vm2 = __ldg(vy + c - 2 * sy), vm1 = __ldg(vy + c - sy), v0 = __ldg(vy + c), vp1 = __ldg(vy + c + sy), vp2 = __ldg(vy + c + 2 * sy);
+        const double czp = flatten_coeff_1d(gamma, pa, pb, pc, pd, pe, wa, wc);       // chi~_z(k+1)
+        const double cxm = flatten_coeff_1d(gamma, xm3, xm2, xm1, pb, xp1, um2, u0);
+        const double cx0 = flatten_coeff_1d(gamma, xm2, xm1, pb, xp1, xp2, um1, up1);
+        const double cxp = flatten_coeff_1d(gamma, xm1, pb, xp1, xp2, xp3, u0, up2);
+        const double cym = flatten_coeff_1d(gamma, ym3, ym2, ym1, pb, yp1, vm2, v0);
+        const double cy0 = flatten_coeff_1d(gamma, ym2, ym1, pb, yp1, yp2, vm1, vp1);
+        const double cyp = flatten_coeff_1d(gamma, ym1, pb, yp1, yp2, yp3, v0, vp2);
+        double x = 1.0;      // same nesting as the oracle: min(1, min(lo, min(mid, hi))) per direction
+        x = lesser(x, lesser(cxm, lesser(cx0, cxp)));
+        x = lesser(x, lesser(cym, lesser(cy0, cyp)));
+        x = lesser(x, lesser(czm, lesser(cz0, czp)));
+        chi[c] = x;
+        pa = pb; pb = pc; pc = pd; pd = pe; wa = wb; wb = wc; czm = cz0; cz0 = czp;
+    }
+}
+
+// chunk length of the flattening march: whole waves of CTAs, long chunks (a chunk's prologue costs about half a step)
+static int chi_len(int nplanes, int ctas_xy, int per_sm)
+{
+    const double per_wave = 148.0 * per_sm;
+    int best = nplanes < 1 ? 1 : nplanes;
+    double best_cost = 1e30;
+    for (int len = 4; len <= 96; ++len) {
+        if (len > nplanes) break;
+        const int chunks = (nplanes + len - 1) / len;
+        const double waves = (double)ctas_xy * chunks / per_wave;
+        const double waves_up = (double)(long long)(waves + 0.999999);
+        const double cost = (1.0 + 0.5 / len) * (waves_up / waves) * ((double)chunks * len / nplanes);
+        if (cost < best_cost - 1e-12) { best_cost = cost; best = len; }
+    }
+    return best;
+}
+
 // chi~_d for the planes [d0, d1) (within [-2, nz+2)), then chi for the planes [m0, m1) (within [-1, nz+1)); an empty
 // range launches nothing.  The whole box is (-2, nz+2, -1, nz+1); a decomposed box does the planes that need no
 // neighbour data first.
 int launch_chi(const Geom &g, double gamma, CHydro5 W, double *cx, double *cy, double *cz, double *chi, int d0, int d1,
-               int m0, int m1, cudaStream_t st)
+               int m0, int m1, int path, cudaStream_t st)
 {
     int n = 0;
+    // path 0: by box size.  Boxes whose three chi~ arrays stay in the 126 MB L2 between the two passes (up to ~160^3)
+    // are faster with the two passes (128^3: 0.054 against 0.071 ms); beyond that the single pass wins (192^3: 0.118
+    // against 0.134 ms, 256^3: 0.250 against 0.290 ms, 320^3: 0.467 against 0.543 ms) and moves half the bytes.
+    if (path == 2 || (path == 0 && 3.0 * 8.0 * (double)g.ntot > 100.0e6)) {
+        if (m1 > m0) {
+            const int bx = (g.nx + 2 + CHI_TX - 1) / CHI_TX, by = (g.ny + 2 + CHI_TY - 1) / CHI_TY;
+            const int len = chi_len(m1 - m0, bx * by, CHI_MINB);
+            dim3 grid(bx, by, (m1 - m0 + len - 1) / len);
+            chi_march_kernel<<<grid, dim3(CHI_TX, CHI_TY), 0, st>>>(g, m0, m1, len, gamma, W.E, W.mx, W.my, W.mz, chi);
+            ++n;
+        }
+        return n;
+    }
     const bool vec = (g.nx & 1) == 0;
     if (d1 > d0) {
         if (vec) {

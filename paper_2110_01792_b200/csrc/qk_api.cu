@@ -44,6 +44,7 @@ struct qk_ctx {
     double *stage[N_STAGE];
     double *chi;
     double *chi3[3];       // directional flattening coefficients
+    int chi_path;          // qk_set_flatten_path
     double *acc[N_ACC];
     double *recon[N_RECON];
     Counters *ctr;
@@ -300,7 +301,7 @@ int hydro_stage(qk_ctx *c, double dtdx, int stage, double *const *U, double *con
     const int nz = g.nz;
     auto chi = [&](int d0, int d1, int m0, int m1) {
         Scope s(c, K_FLATTEN);
-        s.done(launch_chi(g, c->pc.gamma, ch5(W), c->chi3[0], c->chi3[1], c->chi3[2], c->chi, d0, d1, m0, m1, c->stream));
+        s.done(launch_chi(g, c->pc.gamma, ch5(W), c->chi3[0], c->chi3[1], c->chi3[2], c->chi, d0, d1, m0, m1, c->chi_path, c->stream));
     };
     auto sweep = [&](int d, int k0, int k1) {
         Scope s(c, K_HYDRO_X + d);
@@ -487,6 +488,7 @@ int qk_init(int nx, int ny, int nz, double dx, double gamma, double c_hat, doubl
     x->pc.flags = 0;                     // plain HLL: the optical-depth correction is opt-in (R6)
     x->pc.bc = boundary;
     x->stream = nullptr; x->device = dev; x->base = nullptr; x->bytes = 0; x->owns = false; x->ready = false;
+    x->chi_path = 0;
     x->w_cur = 0; x->s_cur = 0; x->w_valid = false; x->s_valid = false; x->smax_valid = false; x->has_source = false; x->has_fixed = boundary == QK_BC_FIXED;
     for (int f = 0; f < 6; ++f) x->fb.t[f] = boundary;
     x->ext_faces = 0; x->halo_fn = nullptr; x->halo_user = nullptr; x->pending.n = 0; x->in_halo_cb = false;
@@ -1003,6 +1005,13 @@ int qk_set_profiling(qk_ctx *c, int on)
 {
     if (!c) return QK_EINVAL;
     c->profiling = on != 0;
+    return QK_OK;
+}
+
+int qk_set_flatten_path(qk_ctx *c, int path)
+{
+    if (!c || path < 0 || path > 2) return QK_EINVAL;
+    c->chi_path = path;
     return QK_OK;
 }
 

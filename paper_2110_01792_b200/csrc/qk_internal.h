@@ -99,7 +99,7 @@ int launch_cfl(const Geom &g, double gamma, CHydro5 U, StateCache *cache, cudaSt
 // U / R: that state (own-cell reads of the update); U0 / R0: the state at the start of the step; Wout / Sout: the
 // reconstruction variables of the updated interior cells.
 int launch_chi(const Geom &g, double gamma, CHydro5 W, double *cx, double *cy, double *cz, double *chi, int d0, int d1,
-               int m0, int m1, cudaStream_t st);
+               int m0, int m1, int path, cudaStream_t st);
 int launch_hydro_sweeps(const Geom &g, double gamma, unsigned scheme, double dtdx, int stage, CHydro5 W,
                         const double *chi, Hydro5 D, CHydro5 U, CHydro5 U0, Hydro5 out, Hydro5 Wout, Counters *ctr,
                         StateCache *cache, cudaStream_t st, int which, const double *dtdx_dev, int k0, int k1);

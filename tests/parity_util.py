@@ -25,7 +25,11 @@ def make_oracle(params, fields):
 
 
 def make_gpu(params, fields, path=None, **kw):
-    return B.from_params(params, fields, **kw)
+    """path: qk_set_flatten_path (1 two passes, 2 one pass; None = the library's choice by box size)"""
+    ctx = B.from_params(params, fields, **kw)
+    if path is not None:
+        ctx.qk_set_flatten_path(path)
+    return ctx
 
 
 def rel_errors(ref: dict, got: dict, groups=None):

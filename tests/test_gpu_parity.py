@@ -16,8 +16,10 @@ import parity_util as P
 
 pytestmark = pytest.mark.gpu
 
-PATHS = [None]          # one stage implementation (the direction-split sweeps); the parameter is kept for the ids
-PATH_IDS = ["sweep"]
+# the two implementations of the flattening coefficient (qk_set_flatten_path): small boxes would only ever run the
+# two-pass one by default, so the hydro parity tests run both on every shape
+PATHS = [1, 2]
+PATH_IDS = ["chi_two_pass", "chi_one_pass"]
 
 
 # ------------------------------------------------------------------------------------------------
@@ -168,19 +170,21 @@ def test_hydro_ragged_shocks(bc, path):
     P.assert_parity(*res[5], P.TOL_100_STEPS, P.HYDRO, "ragged step 5")
 
 
-@pytest.mark.parametrize("shape", [(1, 1, 40), (4, 4, 33), (3, 70, 5), (66, 2, 3), (8, 8, 8)])
-def test_hydro_thin_and_tiny_boxes(shape):
+@pytest.mark.parametrize("path", PATHS, ids=PATH_IDS)
+@pytest.mark.parametrize("shape", [(1, 1, 40), (4, 4, 33), (3, 70, 5), (66, 2, 3), (8, 8, 8), (70, 9, 41)])
+def test_hydro_thin_and_tiny_boxes(shape, path):
     """Degenerate extents (1-3 cells across, where periodic ghosts wrap several times)."""
     params, fields = I.ragged_hydro(shape=shape, seed=5)
-    res = _run_hydro_pair(params, fields, 3, None, check_at=(1,))
+    res = _run_hydro_pair(params, fields, 3, path, check_at=(1,))
     P.assert_parity(*res[1], P.TOL_ONE_STEP, P.HYDRO, "thin %s" % (shape,))
     P.assert_parity(*res[3], P.TOL_100_STEPS, P.HYDRO, "thin %s" % (shape,))
 
 
-def test_hydro_sedov_small_bitwise():
+@pytest.mark.parametrize("path", PATHS, ids=PATH_IDS)
+def test_hydro_sedov_small_bitwise(path):
     """The paper's hydro benchmark problem at 40^3: strong shock from rest."""
     params, fields = I.sedov(n=40)
-    res = _run_hydro_pair(params, fields, 8, None)
+    res = _run_hydro_pair(params, fields, 8, path)
     P.assert_parity(*res[8], P.TOL_100_STEPS, P.HYDRO, "sedov")
     print("sedov mismatching cells:", P.count_mismatch(*res[8], I.FIELDS[:5]))
 
@@ -394,7 +398,7 @@ def test_rhd_step_ragged(bc, path, tau_corr):
     """Full operator-split cycle (hydro, N_sub x (transport, exchange)) on a ragged box."""
     params, fields = I.ragged_rhd(bc=bc, tau_corr=tau_corr)
     g = P.make_oracle(params, fields)
-    with P.make_gpu(params, fields) as ctx:
+    with P.make_gpu(params, fields, path=path) as ctx:
         for s in range(1, 5):
             dt_o, dt_g = g.cfl_dt(), ctx.qk_cfl_dt()
             assert dt_o == dt_g
@@ -643,7 +647,7 @@ def test_slab_decomposition_is_bitwise_the_single_box(kind, world, bc):
         assert sum(p[1]["newton_total_iters"] for p in parts) == info1["newton_total_iters"]
 
 
-def _run_peer_decomposed(params, fields, world, nsteps, kind):
+def _run_peer_decomposed(params, fields, world, nsteps, kind, path=None):
     """`world` slabs as `world` contexts on the one GPU, each on its own stream, driven in lockstep by this one host
     thread through the peer-mapped exchange (qk_halo_export / qk_set_halo_peers): boundary planes are written into the
     neighbour's ghost planes by kernels on side streams, arrival is a stream memory operation -- no callback, no host
@@ -657,7 +661,8 @@ def _run_peer_decomposed(params, fields, world, nsteps, kind):
         k0, nz = D.slab_extent(nzg, rank, world)
         st = torch.cuda.Stream()
         with torch.cuda.stream(st):
-            ctx = P.make_gpu(dict(params, nz=nz), {n: np.ascontiguousarray(a[k0:k0 + nz]) for n, a in fields.items()})
+            ctx = P.make_gpu(dict(params, nz=nz), {n: np.ascontiguousarray(a[k0:k0 + nz]) for n, a in fields.items()},
+                             path=path)
         ctxs.append(ctx)
         streams.append(st)
     handles = [c.qk_halo_export() for c in ctxs]
@@ -679,7 +684,8 @@ def _run_peer_decomposed(params, fields, world, nsteps, kind):
 @pytest.mark.parametrize("kind,world,shape", [("hydro", 2, None), ("hydro", 3, None), ("hydro", 3, (31, 12, 16)),
                                               ("rhd", 2, None), ("rhd", 3, (29, 10, 14))],
                          ids=["hydro2", "hydro3_thin_slabs", "hydro3", "rhd2", "rhd3"])
-def test_peer_mapped_decomposition_is_bitwise_the_single_box(kind, world, shape, bc):
+@pytest.mark.parametrize("path", PATHS, ids=PATH_IDS)
+def test_peer_mapped_decomposition_is_bitwise_the_single_box(kind, world, shape, bc, path):
     """The overlapped in-library exchange: slabs of 8 or more planes run the interior flattening and x / y sweeps while
     the halos travel, thinner slabs wait first; either way the glued result is the single box, bit for bit."""
     gen = I.ragged_hydro if kind == "hydro" else I.ragged_rhd
@@ -691,7 +697,7 @@ def test_peer_mapped_decomposition_is_bitwise_the_single_box(kind, world, shape,
             ctx.qk_hydro_step(dt) if kind == "hydro" else ctx.qk_rhd_step(dt)
         single = ctx.get_all(I.FIELDS[:9])
         info1 = ctx.qk_last_info()
-    parts = _run_peer_decomposed(params, fields, world, nsteps, kind)
+    parts = _run_peer_decomposed(params, fields, world, nsteps, kind, path)
     names = I.FIELDS[:5] if kind == "hydro" else I.FIELDS[:9]
     glued = {n: np.concatenate([parts[r][0][n] for r in range(world)], axis=0) for n in names}
     P.assert_bitwise(single, glued, names, "peer-mapped %s x%d" % (kind, world))
