@@ -286,6 +286,31 @@ int qk_fp64_probe(int kind, int iters, void *cuda_stream, double *lane_ops_per_s
 int qk_selftest_divsqrt(long long n, unsigned long long seed, int exponent_span, void *cuda_stream,
                         long long *out4);
 
+/* ---- Allocation-free entry point -------------------------------------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * it): the hydro timestep of eq 21, dt = cfl * dx / max_cells(|v| + c_s), of a DENSE state, with
+ * no context and no allocation of any kind.  rho, mx, my, mz, E: DEVICE pointers to ncells contiguous doubles each
+ * (conserved variables, any cell order, no ghost cells; read only).  dt_out: DEVICE pointer to one double, written
+ * by the last kernel (NaN if a cell has rho <= 0 or P <= 0).  Asynchronous on cuda_stream (a cudaStream_t; NULL =
+ * the default stream); nothing is read back, nothing synchronises.  The value equals qk_cfl_dt's bit for bit on the
+ * same cells (with c_hat = 0: there is no radiation limit here).
+ * Scratch: one partial maximum per 1024 cells and a bad-cell counter live in a file-scope device array of
+ * QK_NOALLOC_SCRATCH_BYTES that every GPU loading the library holds until exit; hence the limit
+ * ncells <= QK_NOALLOC_MAX_CELLS (256^3), beyond which the call returns QK_ENOMEM and launches nothing.
+ * QK_EINVAL for a null pointer, ncells < 1, gamma <= 1, cfl <= 0 or dx <= 0; QK_ECUDA if a CUDA call fails.
+ * The array is shared by every call in the process and keeps the last call's contents (the call clears the counter
+ * it needs at zero itself): calls that may overlap on the GPU -- different streams, several host threads -- race on
+ * it and must be serialised by the caller.
+ * qk_noalloc_setup resolves the array's device address for the CURRENT device (cudaGetSymbolAddress, once per
+ * device); qk_cfl_dt_noalloc does the same on first use, so calling it is only needed before a region in which
+ * even that query is unwelcome (stream capture).  qk_noalloc_max_cells returns QK_NOALLOC_MAX_CELLS. */
+#define QK_NOALLOC_MAX_CELLS 16777216LL
+#define QK_NOALLOC_SCRATCH_BYTES 131328
+int qk_noalloc_setup(void);
+long long qk_noalloc_max_cells(void);
+int qk_cfl_dt_noalloc(const double *rho, const double *mx, const double *my, const double *mz, const double *E,
+                      long long ncells, double gamma, double cfl, double dx, void *cuda_stream, double *dt_out);
+
 const char *qk_version(void);
 
 #ifdef __cplusplus

@@ -31,6 +31,7 @@ EXPORTS = [
     "qk_selftest_divsqrt", "qk_set_eos", "qk_set_opacity_law", "qk_set_opacity_law_T", "qk_set_face_boundaries",
     "qk_hydro_step_cfl", "qk_rhd_step_cfl", "qk_last_dt", "qk_set_halo_exchange", "qk_halo_doubles", "qk_halo_pack",
     "qk_halo_unpack", "qk_set_state_all", "qk_get_state_all", "qk_wait_copies", "qk_halo_export", "qk_set_halo_peers",
+    "qk_noalloc_setup", "qk_noalloc_max_cells", "qk_cfl_dt_noalloc",
 ]
 
 
@@ -106,6 +107,9 @@ def lib():
         "qk_kernel_times": (i, [p, C.POINTER(d), C.POINTER(ll)]),
         "qk_version": (C.c_char_p, []),
         "qk_fp64_probe": (i, [i, i, p, C.POINTER(d)]),
+        "qk_noalloc_setup": (i, []),
+        "qk_noalloc_max_cells": (ll, []),
+        "qk_cfl_dt_noalloc": (i, [p, p, p, p, p, ll, d, d, d, p, p]),
         "qk_selftest_divsqrt": (i, [ll, C.c_ulonglong, i, p, C.POINTER(ll)]),
         "qk_set_halo_exchange": (i, [p, u, HALO_FN, p]),
         "qk_halo_doubles": (C.c_size_t, [p]),
@@ -129,6 +133,27 @@ def qk_fp64_probe(kind=0, iters=20000):
     _check(lib().qk_fp64_probe(kind, iters, C.c_void_p(torch.cuda.current_stream().cuda_stream), C.byref(out)),
            "qk_fp64_probe")
     return float(out.value)
+
+
+def qk_noalloc_setup():
+    _check(lib().qk_noalloc_setup(), "qk_noalloc_setup")
+
+
+def qk_noalloc_max_cells():
+    return int(lib().qk_noalloc_max_cells())
+
+
+def qk_cfl_dt_noalloc(rho, mx, my, mz, E, ncells, gamma, cfl, dx, dt_out, stream=None):
+    """Allocation-free eq 21 timestep (include/qk.h).  rho..E, dt_out: DEVICE addresses (ints); dt_out receives one
+    double.  Asynchronous on `stream` (a raw cudaStream_t; default: torch's current stream)."""
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream().cuda_stream
+    rc = lib().qk_cfl_dt_noalloc(C.c_void_p(rho), C.c_void_p(mx), C.c_void_p(my), C.c_void_p(mz), C.c_void_p(E),
+                                 int(ncells), float(gamma), float(cfl), float(dx), C.c_void_p(stream), C.c_void_p(dt_out))
+    if rc == QK_ENOMEM:
+        raise QkError("qk_cfl_dt_noalloc: %d cells exceed the fixed scratch's limit of %d" % (ncells, qk_noalloc_max_cells()))
+    _check(rc, "qk_cfl_dt_noalloc")
 
 
 def qk_selftest_divsqrt(n, seed=1, exponent_span=2046):

@@ -20,7 +20,7 @@ INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libqk.so")
 OBJ = os.path.join(HERE, "build")
 
-SOURCES = ["qk_api.cu", "k_boundary.cu", "k_cfl.cu", "k_exchange.cu", "k_sweep.cu", "k_peak.cu"]
+SOURCES = ["qk_api.cu", "k_boundary.cu", "k_cfl.cu", "k_exchange.cu", "k_sweep.cu", "k_peak.cu", "k_noalloc.cu"]
 HEADERS = ["qk_internal.h", "qk_math.cuh", "qk_fastmath.cuh", "k_recon.cuh", "k_sweep.cuh"]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-fmad=false",

@@ -38,7 +38,8 @@ def test_binding_has_every_entry_point():
     for n in _declared():
         assert n in B.EXPORTS
         if n not in ("qk_init", "qk_free", "qk_state_bytes", "qk_bind_storage", "qk_version",
-                     "qk_kernel_class_count", "qk_kernel_class_name", "qk_fp64_probe", "qk_selftest_divsqrt"):
+                     "qk_kernel_class_count", "qk_kernel_class_name", "qk_fp64_probe", "qk_selftest_divsqrt",
+                     "qk_noalloc_setup", "qk_noalloc_max_cells", "qk_cfl_dt_noalloc"):
             assert hasattr(B.Context, n), n
 
 
