@@ -316,6 +316,21 @@ struct ExchangeConsts {
     bool literal_stop, static_matter;
 };
 
+// The decision |x / y| < tol of eq 36-37, taken without the division wherever it cannot matter: with
+// b = fl(tol |y|) = tol |y| (1 + d), |d| <= 2^-53 (b normal), |x| < b/2 implies fl(|x|/|y|) <= tol (1 + d)(1 + d')/2 < tol
+// and |x| > 2b implies fl(|x|/|y|) >= 2 tol (1 - 2^-52) > tol (rounding is monotone); only inside the factor-4 band
+// around the threshold -- or when b is not a normal positive number (y zero, tiny, NaN; tol <= 0) -- is the quotient
+// formed.  Same decision as fabs(x / y) < tol for every input; saves two of the seven divisions of a Newton iteration.
+QK_HD bool below_tolerance(double x, double y, double tol)
+{
+    const double a = fabs(x), b = tol * fabs(y);
+    if (b >= 1e-290) {
+        if (a < 0.5 * b) return true;
+        if (a > 2.0 * b) return false;
+    }
+    return fabs(x / y) < tol;
+}
+
 // Backward-Euler update of one cell over dt.  In/out: m (gas momentum), E, Er, F.  Returns 0,
 // 4 (Newton cap reached) or 5 (non-positive E_g or E_r afterwards); iters = Newton updates.
 template <bool KT>
@@ -355,7 +370,7 @@ QK_HD int exchange_cell(const ExchangeConsts &k, double dt, double rho, double &
         const double R = coef * (k.a_rad * T4 - Erad);                    // eq 28 (X1)
         const double FG = (Eg - Eg_old) + c_ratio * R;                    // eq 26
         const double FR = (Erad - Er_old) - (R + S);                      // eq 27
-        const bool converged = (fabs(FG / Etot) < k.tol) && (fabs(c_ratio * FR / Etot) < k.tol);  // eq 36-37
+        const bool converged = below_tolerance(FG, Etot, k.tol) && below_tolerance(c_ratio * FR, Etot, k.tol);  // eq 36-37
         if (converged && k.literal_stop) { finished = true; break; }
         double dR_dEg = coef * (4.0 * k.a_rad * (T2 * T)) / Cv;           // eq 33 with d kappa/dT = 0
         if (KT) dR_dEg = (coef * (4.0 * k.a_rad * (T2 * T)) + dcoef_dT * (k.a_rad * T4 - Erad)) / Cv;   // eq 33
