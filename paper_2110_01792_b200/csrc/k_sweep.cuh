@@ -151,19 +151,21 @@ __global__ void __launch_bounds__(SW_NT, PH::X_MINB) sweep_x_kernel(PH ph, Geom 
 // ---- y and z sweeps: marching columns ----------------------------------------------------------------------
 // DIR = 1: march along y (blockIdx.y = k), D += dF_y.  DIR = 2: march along z (blockIdx.y = j), RK stage update
 // from (dF_x + dF_y) + dF_z (the paper's sum order).
-template <class PH, int DIR>
-__global__ void __launch_bounds__(SW_NT, DIR == 2 ? PH::Z_MINB : PH::Y_MINB) sweep_march_kernel(PH ph, Geom g, int len, int o0, FieldsRW<PH::NV> D, RkArgs rk,
+// NT = threads per CTA = columns along x per CTA (128, 64 or 32: the launcher takes the width that wastes the fewest
+// lanes on the row length; the CTAs per SM scale with 128 / NT, so the resident warps stay the same)
+template <class PH, int DIR, int NT>
+__global__ void __launch_bounds__(NT, (DIR == 2 ? PH::Z_MINB : PH::Y_MINB) * (SW_NT / NT)) sweep_march_kernel(PH ph, Geom g, int len, int o0, FieldsRW<PH::NV> D, RkArgs rk,
                                                                    FieldsRO<PH::NV> U, FieldsRO<PH::NV> U0, FieldsRW<PH::NV> out,
                                                                    FieldsRW<PH::NV> pout, Counters *ctr, StateCache *cache)
 {
     constexpr int NV = PH::NV;
     const double dtdx = (DIR == 2 && rk.dtdx_dev) ? __ldg(rk.dtdx_dev) : rk.dtdx;
     typename PH::Tail tail;                             // per-thread reduction state of the z epilogue
-    __shared__ double ring[5 * SW_NR * SW_NT];          // [slot][var][thread], thread-private columns
+    __shared__ double ring[5 * SW_NR * NT];          // [slot][var][thread], thread-private columns
     // own-cell inputs of the update (D; for z also U and U^n), staged global -> shared by cp.async: [array][var][thread]
-    __shared__ double own[(DIR == 2 ? 3 : 1) * PH::NV * SW_NT];   // z: D, U, U^n of the cell being updated, staged by cp.async
+    __shared__ double own[(DIR == 2 ? 3 : 1) * PH::NV * NT];   // z: D, U, U^n of the cell being updated, staged by cp.async
     const int tid = threadIdx.x;
-    const int i = blockIdx.x * SW_NT + tid;
+    const int i = blockIdx.x * NT + tid;
     const bool active = i < g.nx;
     const int o = (int)blockIdx.y + o0;                 // y sweep: the launch covers the planes o0 .. o0 + gridDim.y - 1
     const int n_m = DIR == 1 ? g.ny : g.nz;
@@ -174,8 +176,8 @@ __global__ void __launch_bounds__(SW_NT, DIR == 2 ? PH::Z_MINB : PH::Y_MINB) swe
     const int base = DIR == 1 ? g.at(ic, 0, o) : g.at(ic, o, 0);     // cell m = 0 of the column
 
     // rotating ring offsets of the cells m-1, m, m+1, m+2, m+3
-    int r0 = 0 * SW_NR * SW_NT + tid, r1 = 1 * SW_NR * SW_NT + tid, r2 = 2 * SW_NR * SW_NT + tid,
-        r3 = 3 * SW_NR * SW_NT + tid, r4 = 4 * SW_NR * SW_NT + tid;
+    int r0 = 0 * SW_NR * NT + tid, r1 = 1 * SW_NR * NT + tid, r2 = 2 * SW_NR * NT + tid,
+        r3 = 3 * SW_NR * NT + tid, r4 = 4 * SW_NR * NT + tid;
     // prologue: cells m0-3..m0 -> r0..r3 (they are cells m-1..m+2 of the first step m = m0-2)
     {
         const int rr[4] = {r0, r1, r2, r3};
@@ -183,7 +185,7 @@ __global__ void __launch_bounds__(SW_NT, DIR == 2 ? PH::Z_MINB : PH::Y_MINB) swe
         for (int p = 0; p < 4; ++p) {
             const int cidx = base + (m0 - 3 + p) * s;
 #pragma unroll
-            for (int v = 0; v < SW_NR; ++v) ring[rr[p] + v * SW_NT] = ph.ld(v, cidx);
+            for (int v = 0; v < SW_NR; ++v) ring[rr[p] + v * NT] = ph.ld(v, cidx);
         }
     }
     double pend[SW_NR];
@@ -195,13 +197,13 @@ __global__ void __launch_bounds__(SW_NT, DIR == 2 ? PH::Z_MINB : PH::Y_MINB) swe
     for (int v = 0; v < NV; ++v) {
         hiP[v] = 0.0; Flo[v] = 0.0;
         // raw eq 22 interface at the low face of the first cell reconstructed (cells m0-3..m0 are in r0..r3)
-        ifc[v] = ppm_interface(ring[r0 + v * SW_NT], ring[r1 + v * SW_NT], ring[r2 + v * SW_NT], ring[r3 + v * SW_NT]);
+        ifc[v] = ppm_interface(ring[r0 + v * NT], ring[r1 + v * NT], ring[r2 + v * NT], ring[r3 + v * NT]);
     }
     int nfall = 0, nguard = 0;
 
     for (int m = m0 - 2; m < m1; ++m) {
 #pragma unroll
-        for (int v = 0; v < SW_NR; ++v) ring[r4 + v * SW_NT] = pend[v];
+        for (int v = 0; v < SW_NR; ++v) ring[r4 + v * NT] = pend[v];
         const double aux = aux_next;
         if (m + 1 < m1) {
             const int cn = base + (m + 4) * s;
@@ -215,10 +217,10 @@ __global__ void __launch_bounds__(SW_NT, DIR == 2 ? PH::Z_MINB : PH::Y_MINB) swe
             {     // global -> shared without passing through registers: they land while the Riemann solve runs
 #pragma unroll
                 for (int v = 0; v < NV; ++v) {
-                    cp_async8(&own[(0 * NV + v) * SW_NT + tid], D.f[v] + cidx);
+                    cp_async8(&own[(0 * NV + v) * NT + tid], D.f[v] + cidx);
                     if (DIR == 2) {
-                        cp_async8(&own[(1 * NV + v) * SW_NT + tid], U.f[v] + cidx);
-                        if (rk.stage == 1) cp_async8(&own[(2 * NV + v) * SW_NT + tid], U0.f[v] + cidx);
+                        cp_async8(&own[(1 * NV + v) * NT + tid], U.f[v] + cidx);
+                        if (rk.stage == 1) cp_async8(&own[(2 * NV + v) * NT + tid], U0.f[v] + cidx);
                     }
                 }
                 cp_async_commit();
@@ -228,14 +230,14 @@ __global__ void __launch_bounds__(SW_NT, DIR == 2 ? PH::Z_MINB : PH::Y_MINB) swe
         double lo[NV], hi[NV], Fhi[NV];
         {
             const int rr[5] = {r0, r1, r2, r3, r4};
-            const auto win = [&](int v, int q) { return ring[rr[q] + v * SW_NT]; };
+            const auto win = [&](int v, int q) { return ring[rr[q] + v * NT]; };
             const int nf = PH::CARRY ? ph.template states_carry<PH::BL_MARCH>(win, aux, ifc, lo, hi)
                                      : ph.template states<PH::BL_MARCH>(win, aux, lo, hi);
             const int mm = m + 1;
             if (PH::COUNTS && active && ((mm >= m0 && mm < m1) || mm == -1 || mm == n_m)) nfall += nf;
         }
         if (m >= m0 - 1) {      // face m+1/2 = low face of cell m+1
-            const int gd = ph.template flux<DIR>(hiP, lo, ring[r1 + (SW_NR - 1) * SW_NT], ring[r2 + (SW_NR - 1) * SW_NT], Fhi);
+            const int gd = ph.template flux<DIR>(hiP, lo, ring[r1 + (SW_NR - 1) * NT], ring[r2 + (SW_NR - 1) * NT], Fhi);
             const int mm = m + 1;
             if (PH::COUNTS && active && ((mm >= m0 && mm < m1) || mm == n_m)) nguard += gd;
         }
@@ -244,13 +246,13 @@ __global__ void __launch_bounds__(SW_NT, DIR == 2 ? PH::Z_MINB : PH::Y_MINB) swe
             double fresh[NV];
 #pragma unroll
             for (int v = 0; v < NV; ++v) {
-                const double dv = own[(0 * NV + v) * SW_NT + tid];
+                const double dv = own[(0 * NV + v) * NT + tid];
                 const double div = dv + (Fhi[v] - Flo[v]);                  // dF_x + dF_y, then (dF_x + dF_y) + dF_z
                 if (DIR == 1) {
                     D.f[v][cidx] = div;
                 } else {
-                    const double us = own[(1 * NV + v) * SW_NT + tid] - dtdx * div;
-                    fresh[v] = rk.stage == 0 ? us : 0.5 * own[(2 * NV + v) * SW_NT + tid] + 0.5 * us;
+                    const double us = own[(1 * NV + v) * NT + tid] - dtdx * div;
+                    fresh[v] = rk.stage == 0 ? us : 0.5 * own[(2 * NV + v) * NT + tid] + 0.5 * us;
                     out.f[v][cidx] = fresh[v];
                 }
             }
