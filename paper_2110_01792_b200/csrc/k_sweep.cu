@@ -315,6 +315,8 @@ __global__ void __launch_bounds__(128) chi_min2_kernel(Geom g, int k0, const dou
 // spills) 0.275 ms, 32 x 2 at 10: 0.253 ms; grouping the loads by direction instead of issuing all 24 first: 0.35 ms.
 constexpr int CHI_TX = 32, CHI_TY = 4, CHI_MINB = 5;
 
+__device__ __forceinline__ void prefetch_l2(const double *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
 __global__ void __launch_bounds__(CHI_TX * CHI_TY, CHI_MINB) chi_march_kernel(Geom g, int m0, int m1, int len, double gamma,
                                                                     const double *__restrict__ P, const double *__restrict__ vx,
                                                                     const double *__restrict__ vy, const double *__restrict__ vz,
@@ -339,6 +341,12 @@ __global__ void __launch_bounds__(CHI_TX * CHI_TY, CHI_MINB) chi_march_kernel(Ge
     for (int k = ka; k < kb; ++k, c += sz) {
         // all 24 loads of the step are issued before the first evaluation: the kernel lives on memory-level parallelism
         const double pe = __ldg(P + c + 3 * sz), wc = __ldg(vz + c + 2 * sz);
+        // the four lines of this column's data that the step two planes on touches for the first time, asked into the
+        // L2 now (no register, no dependency): its loads then miss the L1 only as far as the L2 (0.254 -> 0.235 ms)
+        if (k + 2 < kb) {
+            const int cp = c + 2 * sz;
+            prefetch_l2(P + cp + 3 * sz); prefetch_l2(vz + cp + 2 * sz); prefetch_l2(vx + cp); prefetch_l2(vy + cp);
+        }
         const double xm3 = __ldg(P + c - 3), xm2 = __ldg(P + c - 2), xm1 = __ldg(P + c - 1);
         const double xp1 = __ldg(P + c + 1), xp2 = __ldg(P + c + 2), xp3 = __ldg(P + c + 3);
         const double um2 = __ldg(vx + c - 2), um1 = __ldg(vx + c - 1), u0 = __ldg(vx + c), up1 = __ldg(vx + c + 1), up2 = __ldg(vx + c + 2);
