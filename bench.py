@@ -16,7 +16,8 @@ HOST buffers: every step uploads the evolving fields from pinned memory (qk_set_
 (qk_get_state_all), all inside the timed region, with three boxes in flight so that upload, step and download
 overlap.  Working set per step (5 x 147 MB read, plus stage buffers) is several times the 126 MB L2, so no
 explicit flush is needed.  The same JSON line carries sub-records for the other BASELINE configs: "rhd"
-(configs[3]), "rad" (configs[2], 128^3), "size512" (configs[4]) and "rhd_nsub10" (the paper's N_sub = 10 shape).
+(configs[3]), "rad" (configs[2], 128^3), "size512" (configs[4]), "rhd_nsub10" (the paper's N_sub = 10 shape) and
+"small_boxes" (launch-bound sizes: ordinary step, device-resident timestep, replayed CUDA graph).
 
 --impl reference times the CPU oracle (oracle/, plain C, its loops dealt out to the host's cores) on a bounded
 sample of the same workload; it is a deliberately slow baseline.
@@ -380,6 +381,33 @@ def run_workload(torch, B, I, kind, params, fields, steps, warmup, rank, world, 
     return out
 
 
+def small_box_record(torch, B, I, sizes, steps=200):
+    """Boxes whose step is bound by launch overhead (BASELINE configs[0] is 32^3): the hydro step with the host
+    timestep, with the device-resident timestep, and as a replayed CUDA graph (qk_graph_capture / qk_graph_launch),
+    all on a side stream (the legacy default stream cannot be captured)."""
+    out = {}
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        for n in sizes:
+            p, f = I.config1(n=n)
+            cells = n ** 3
+            rec = {}
+            with B.from_params(p, f) as ctx:
+                def host_dt():
+                    ctx.qk_hydro_step(ctx.qk_cfl_dt())
+                ctx.qk_graph_capture(B.QK_GRAPH_HYDRO)
+                for label, fn in (("host_dt", host_dt), ("device_dt", ctx.qk_hydro_step_cfl),
+                                  ("graph", lambda: ctx.qk_graph_launch(1))):
+                    ctx.set_all({k: f[k] for k in I.FIELDS[:5]})
+                    for _ in range(5):
+                        fn()
+                    ms = time_loop(torch, fn, steps, lambda: None)
+                    assert ctx.qk_last_info()["status"] == 0
+                    rec[label] = {"value": cells * steps / (ms * 1e-3), "unit": UNIT, "ms_per_step": ms / steps}
+            out["%d^3" % n] = rec
+    return out
+
+
 def roofline_alu(kernel_ms, names, ops_per_cell_per_launch, cells, peak_ops, peak_note):
     """Dominant ALU-bound kernel: algorithmic fp64 ops per launch / mean launch duration."""
     present = [nm for nm in names if nm in kernel_ms]
@@ -517,6 +545,10 @@ def run_ours(args):
                         "kernel_ms": {k: {"total_ms": v[0], "groups": v[1]} for k, v in r["kernel_ms"].items()},
                         "status": r["info"]["status"]}
         del p, f
+        # ---- launch-bound boxes: ordinary step, device-resident timestep, replayed CUDA graph -------------------
+        extra["small_boxes"] = {"config": {"workload": "BASELINE.json configs[0] (32^3) and its generator at 64^3, 128^3: qk_cfl_dt + qk_hydro_step, "
+                                                       "qk_hydro_step_cfl, and qk_graph_launch(1) per step (200 steps each)"},
+                                **small_box_record(torch, B, I, (32, 64, 128))}
         # ---- BASELINE configs[4]: 512^3 ---------------------------------------------------------------------
         if not args.no_512:
             p, f = gen("rhd", 512)

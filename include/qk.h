@@ -234,6 +234,27 @@ int qk_last_dt(qk_ctx *ctx, double *dt);
  * that pair would take nsub substeps of the same dt. */
 int qk_rhd_step_cfl(qk_ctx *ctx, int nsub);
 
+/* Replayable step: ONE qk_hydro_step_cfl (kind QK_GRAPH_HYDRO) or ONE qk_rhd_step_cfl(nsub) (kind QK_GRAPH_RHD)
+ * recorded as a CUDA graph and replayed with one launch per step.  The launch sequence of a step is fixed by the
+ * host-side parameters alone (the timestep of eq 21 stays on the device), so the recorded step is
+ * the same kernels with the same arguments as the ordinary call: results are bit-identical.  For boxes below ~128^3 the
+ * step is bound by launch overhead and the replay removes it.
+ * qk_graph_capture records the steady-state sequence on the context's stream, which must not be the legacy default
+ * stream (QK_EINVAL: it cannot be captured); nothing is executed and the state is not touched.  It replaces an
+ * earlier recording.  QK_EINVAL also for a context with inter-rank faces (see qk_hydro_step_cfl) or with kernel-class
+ * timing on.  Allocation happens here (graph instantiation), never in qk_graph_launch.
+ * qk_graph_launch enqueues `nsteps` steps.  A step whose starting state has no cached reconstruction variables
+ * (the first step after qk_set_state / qk_set_raw) is taken by the ordinary call instead, which builds them.
+ * QK_EINVAL if nothing was recorded or if parameters, boundary types, opacity law, equation of state, source field,
+ * flattening path, storage or stream have changed since the recording: record again.  Counters (qk_last_info) are
+ * those of the last step; qk_last_dt returns its dt.
+ * qk_graph_free drops the recording (qk_free does too). */
+#define QK_GRAPH_HYDRO 0
+#define QK_GRAPH_RHD 1
+int qk_graph_capture(qk_ctx *ctx, int kind, int nsub);
+int qk_graph_launch(qk_ctx *ctx, int nsteps);
+int qk_graph_free(qk_ctx *ctx);
+
 /* SSP-RK2 explicit transport of (E_r, F_r) over dt, no exchange. */
 int qk_rad_transport(qk_ctx *ctx, double dt);
 

@@ -32,6 +32,7 @@ EXPORTS = [
     "qk_hydro_step_cfl", "qk_rhd_step_cfl", "qk_last_dt", "qk_set_halo_exchange", "qk_halo_doubles", "qk_halo_pack",
     "qk_halo_unpack", "qk_set_state_all", "qk_get_state_all", "qk_wait_copies", "qk_halo_export", "qk_set_halo_peers",
     "qk_noalloc_setup", "qk_noalloc_max_cells", "qk_cfl_dt_noalloc",
+    "qk_graph_capture", "qk_graph_launch", "qk_graph_free",
 ]
 
 
@@ -48,6 +49,7 @@ class qk_halo_handle(C.Structure):
 
 QK_FACE_ZLO, QK_FACE_ZHI = 1, 2
 QK_EOS_IDEAL, QK_EOS_ALPHA_T3 = 0, 1
+QK_GRAPH_HYDRO, QK_GRAPH_RHD = 0, 1
 HALO_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_int)
 
 
@@ -93,6 +95,9 @@ def lib():
         "qk_hydro_step_cfl": (i, [p]),
         "qk_rhd_step_cfl": (i, [p, i]),
         "qk_last_dt": (i, [p, C.POINTER(d)]),
+        "qk_graph_capture": (i, [p, i, i]),
+        "qk_graph_launch": (i, [p, i]),
+        "qk_graph_free": (i, [p]),
         "qk_rad_transport": (i, [p, d]),
         "qk_exchange": (i, [p, d]),
         "qk_rad_step": (i, [p, d]),
@@ -343,6 +348,15 @@ class Context:
 
     def qk_rhd_step_cfl(self, nsub):
         _check(self.L.qk_rhd_step_cfl(self.h, nsub), "qk_rhd_step_cfl")
+
+    def qk_graph_capture(self, kind, nsub=0):
+        _check(self.L.qk_graph_capture(self.h, kind, nsub), "qk_graph_capture")
+
+    def qk_graph_launch(self, nsteps=1):
+        _check(self.L.qk_graph_launch(self.h, nsteps), "qk_graph_launch")
+
+    def qk_graph_free(self):
+        _check(self.L.qk_graph_free(self.h), "qk_graph_free")
 
     def qk_last_dt(self):
         out = C.c_double()

@@ -77,6 +77,13 @@ struct qk_ctx {
     cudaEvent_t ev_copy, ev_compute;
     long long launches;
     int last_nsub;
+    // replayable step (qk_graph_capture): the instantiated CUDA graph of one step and everything host-side that its
+    // launch sequence and kernel arguments were derived from -- a launch with another signature is refused
+    struct StepGraph {
+        cudaGraphExec_t exec;
+        int kind, nsub, launches;
+        PhysConsts pc; FaceBc fb; bool has_fixed, has_source; int chi_path; cudaStream_t stream; void *base;
+    } graph;
     // per-kernel-class event timing
     bool profiling;
     struct Span { int cls; cudaEvent_t a, b; };
@@ -497,6 +504,7 @@ int qk_init(int nx, int ny, int nz, double dx, double gamma, double c_hat, doubl
     for (int p = 0; p < 2; ++p) { x->peer[p].base = nullptr; x->peer[p].flag = nullptr; x->peer[p].ipc_ptr = nullptr; x->peer[p].fs = 0; }
     x->copy_stream = nullptr; x->ev_copy = nullptr; x->ev_compute = nullptr;
     x->launches = 0; x->last_nsub = 0; x->profiling = false;
+    x->graph.exec = nullptr;
     *out = x;
     return QK_OK;
 }
@@ -514,6 +522,7 @@ int qk_free(qk_ctx *c)
     if (c->side) { cudaStreamSynchronize(c->side); cudaStreamDestroy(c->side); }
     if (c->ev_main) cudaEventDestroy(c->ev_main);
     if (c->ev_side) cudaEventDestroy(c->ev_side);
+    if (c->graph.exec) cudaGraphExecDestroy(c->graph.exec);
     if (c->owns && c->base) cudaFree(c->base);
     delete c;
     return QK_OK;
@@ -915,6 +924,78 @@ int qk_last_dt(qk_ctx *c, double *dt)
     if (cudaMemcpyAsync(&h, c->ddt, sizeof(h), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
         cudaStreamSynchronize(c->stream) != cudaSuccess) { cudaGetLastError(); return QK_ECUDA; }
     *dt = h.dt;
+    return QK_OK;
+}
+
+// ---- replayable step: one qk_hydro_step_cfl / qk_rhd_step_cfl recorded as a CUDA graph ------------------------
+// The launch sequence of a step depends on the host-side state only (parameters, boundary types, which caches are
+// valid), never on device data -- the timestep stays on the device -- so a step recorded once in the steady state
+// (reconstruction variables and CFL speed left by the previous step) is the step, whatever the data.
+int qk_graph_free(qk_ctx *c)
+{
+    if (!c) return QK_EINVAL;
+    if (c->graph.exec) { cudaGraphExecDestroy(c->graph.exec); c->graph.exec = nullptr; }
+    return QK_OK;
+}
+
+int qk_graph_capture(qk_ctx *c, int kind, int nsub)
+{
+    if (!c || (kind != QK_GRAPH_HYDRO && kind != QK_GRAPH_RHD)) return QK_EINVAL;
+    if (kind == QK_GRAPH_RHD && (nsub < 1 || nsub > c->pc.nsub_max || !(c->pc.c_hat > 0.0) || !(c->pc.c > 0.0))) return QK_EINVAL;
+    if (c->ext_faces || c->profiling || c->halo_failed) return QK_EINVAL;
+    int rc = ensure_storage(c);
+    if (rc) return rc;
+    qk_graph_free(c);
+    // record the steady-state sequence: as if the previous step had left its caches (a launch on a context whose
+    // caches are not valid takes one ordinary step instead, qk_graph_launch)
+    const bool w = c->w_valid, sv = c->s_valid, sm = c->smax_valid;
+    const long long launches0 = c->launches;
+    const int nsub0 = c->last_nsub;
+    c->w_valid = c->s_valid = c->smax_valid = true;
+    if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+        cudaGetLastError();                      // e.g. the legacy default stream cannot be captured
+        c->w_valid = w; c->s_valid = sv; c->smax_valid = sm;
+        return QK_EINVAL;
+    }
+    rc = kind == QK_GRAPH_HYDRO ? qk_hydro_step_cfl(c) : qk_rhd_step_cfl(c, nsub);
+    cudaGraph_t g = nullptr;
+    const cudaError_t e = cudaStreamEndCapture(c->stream, &g);
+    const int per_step = (int)(c->launches - launches0);
+    c->w_valid = w; c->s_valid = sv; c->smax_valid = sm; c->launches = launches0; c->last_nsub = nsub0;
+    if (rc != QK_OK || e != cudaSuccess || !g) {
+        if (g) cudaGraphDestroy(g);
+        cudaGetLastError();
+        return rc != QK_OK ? rc : QK_ECUDA;
+    }
+    cudaGraphExec_t exec = nullptr;
+    const cudaError_t ei = cudaGraphInstantiate(&exec, g, 0);
+    cudaGraphDestroy(g);
+    if (ei != cudaSuccess) { cudaGetLastError(); return QK_ECUDA; }
+    c->graph.exec = exec; c->graph.kind = kind; c->graph.nsub = kind == QK_GRAPH_RHD ? nsub : 0; c->graph.launches = per_step;
+    c->graph.pc = c->pc; c->graph.fb = c->fb; c->graph.has_fixed = c->has_fixed; c->graph.has_source = c->has_source;
+    c->graph.chi_path = c->chi_path; c->graph.stream = c->stream; c->graph.base = c->base;
+    return QK_OK;
+}
+
+int qk_graph_launch(qk_ctx *c, int nsteps)
+{
+    if (!c || !c->graph.exec || nsteps < 0) return QK_EINVAL;
+    const qk_ctx::StepGraph &G = c->graph;
+    // recorded for other parameters, boundaries, storage or stream than the context has now: record again
+    if (memcmp(&G.pc, &c->pc, sizeof(PhysConsts)) != 0 || memcmp(&G.fb, &c->fb, sizeof(FaceBc)) != 0 ||
+        G.has_fixed != c->has_fixed || G.has_source != c->has_source || G.chi_path != c->chi_path ||
+        G.stream != c->stream || G.base != c->base || c->ext_faces || c->profiling || c->halo_failed) return QK_EINVAL;
+    for (int n = 0; n < nsteps; ++n) {
+        const bool steady = c->smax_valid && (c->has_fixed || (c->w_valid && (G.kind == QK_GRAPH_HYDRO || c->s_valid)));
+        if (!steady) {                           // fresh state: the ordinary step builds the caches the graph starts from
+            const int rc = G.kind == QK_GRAPH_HYDRO ? qk_hydro_step_cfl(c) : qk_rhd_step_cfl(c, G.nsub);
+            if (rc) return rc;
+            continue;
+        }
+        if (cudaGraphLaunch(G.exec, c->stream) != cudaSuccess) { cudaGetLastError(); return QK_ECUDA; }
+        c->launches += G.launches;
+        c->last_nsub = G.nsub;
+    }
     return QK_OK;
 }
 
