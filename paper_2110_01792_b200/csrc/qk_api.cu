@@ -472,7 +472,7 @@ void ensure_speed(qk_ctx *c)
 // =================================================================================================
 extern "C" {
 
-const char *qk_version(void) { return "quokka-b200 0.3 (sm_100a, fp64, -fmad=false)"; }
+const char *qk_version(void) { return "quokka-b200 0.4 (sm_100a, fp64, -fmad=false)"; }
 
 int qk_init(int nx, int ny, int nz, double dx, double gamma, double c_hat, double c, int boundary, qk_ctx **out)
 {
