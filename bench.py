@@ -361,6 +361,8 @@ def run_workload(torch, B, I, kind, params, fields, steps, warmup, rank, world, 
             fn = ctx.qk_hydro_step_cfl if kind == "hydro" else (lambda: ctx.qk_rhd_step_cfl(nsub))
             for _ in range(2):
                 fn()
+            ctx.set_all(fields)                    # the same steps 1..K of the config as the headline loop
+            torch.cuda.synchronize()
             ms_d = allmax(time_loop(torch, fn, steps, barrier))
             out["device_dt"] = {"value": world * cells * steps / (ms_d * 1e-3), "unit": UNIT, "ms_per_step": ms_d / steps,
                                 "call": "qk_hydro_step_cfl" if kind == "hydro" else "qk_rhd_step_cfl(%d)" % nsub}
