@@ -91,18 +91,23 @@ __global__ void __launch_bounds__(256) fill_ghost_kernel(Geom g, FaceBc fb, unsi
             continue;
         }
         if (src == dst) continue;
+        // all loads of the cell are issued before its first store (a store between two loads would order them: the
+        // fields may alias as far as the compiler knows, and the kernel lives on loads in flight)
+        double v[QK_NFIELDS];
+#pragma unroll
+        for (int f = 0; f < QK_NFIELDS; ++f)
+            if (f < fl.n) v[f] = fl.f[f][src];
         if (out_refl[0] || out_refl[1] || out_refl[2]) {
             // the normal component of rho v / v / F_r / f changes sign across each wall the image lies beyond
-#pragma unroll 1
-            for (int f = 0; f < fl.n; ++f) {
-                const double v = fl.f[f][src];
+#pragma unroll
+            for (int f = 0; f < QK_NFIELDS; ++f) {
                 const int cm = fl.comp[f];
-                fl.f[f][dst] = (cm >= 0 && out_refl[cm]) ? -v : v;
+                if (f < fl.n && cm >= 0 && out_refl[cm]) v[f] = -v[f];
             }
-            continue;
         }
-#pragma unroll 1
-        for (int f = 0; f < fl.n; ++f) fl.f[f][dst] = fl.f[f][src];
+#pragma unroll
+        for (int f = 0; f < QK_NFIELDS; ++f)
+            if (f < fl.n) fl.f[f][dst] = v[f];
     }
 }
 
