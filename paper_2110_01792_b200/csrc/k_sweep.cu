@@ -34,13 +34,16 @@ template <int RECON>
 struct HydroPhT {
     static constexpr int NV = 5, NSRC = 6;
     static constexpr bool COUNTS = false;
-    // select-only PPM limiter (same values): measured faster in the x sweep, slower in the marching sweeps
-    static constexpr int BL_X = 1, BL_MARCH = 0;
+    // PPM limiter with branches in every sweep.  The select-only form (same values) was faster in the x sweep while its
+    // division chains still branched; since the operand-window Riemann solver and the 16-byte row staging the x sweep is
+    // bound by instruction issue and the fp64 pipe, and the branches skip the MC slope of every cell that is no
+    // extremum: 0.712 -> 0.637 ms at 256^3 (lock-step form: 0.69 ms)
+    static constexpr int BL_X = 0, BL_MARCH = 0;
     static constexpr bool CARRY = true;    // marching sweeps carry the raw interface value (measured: -1.5 %)
     // CTAs per SM.  z runs at 4 (126 registers, no spill) only because its update inputs are staged by cp.async and
     // never sit in registers during the Riemann solve: 0.81 -> 0.77 ms; with register loads 4 CTAs spill (1.10 ms).
-    // y at 5 (96 registers) spills: 0.62 -> 0.78 ms.  x at 6 (78 registers): no gain, it is pipe-bound.
-    static constexpr int X_MINB = 5, Y_MINB = 4, Z_MINB = 4;
+    // y at 5 (96 registers) spills: 0.62 -> 0.78 ms.  x at 6 (78 registers, no spill): 0.637 -> 0.627 ms.
+    static constexpr int X_MINB = 6, Y_MINB = 4, Z_MINB = 4;
     const double *w[5];        // rho, vx, vy, vz, P (ghost cells included)
     const double *chi;         // flattening coefficient of the cells -1..n
     double gamma;
