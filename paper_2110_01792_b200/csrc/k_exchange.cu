@@ -47,10 +47,10 @@ __global__ void __launch_bounds__(128, KT ? 5 : QK_EX_MINB) exchange_kernel(Geom
             cell_prim_speed(kc.gamma, rho[cidx], m0, m1, m2, e, true, p, sp);
             if (!(p.rho > 0.0) || !(p.P > 0.0)) bad_hydro = 1;
             else smax = sp;
-            if (Wout.rho) {
-                Wout.rho[cidx] = p.rho; Wout.mx[cidx] = p.vx; Wout.my[cidx] = p.vy; Wout.mz[cidx] = p.vz; Wout.E[cidx] = p.P;
+            if (Wout.mx) {        // rho and E_r are read from the state by the next stage: not stored again
+                Wout.mx[cidx] = p.vx; Wout.my[cidx] = p.vy; Wout.mz[cidx] = p.vz; Wout.E[cidx] = p.P;
                 const double cE = kc.c * er;
-                Sout.E[cidx] = er; Sout.Fx[cidx] = f0 / cE; Sout.Fy[cidx] = f1 / cE; Sout.Fz[cidx] = f2 / cE;
+                Sout.Fx[cidx] = f0 / cE; Sout.Fy[cidx] = f1 / cE; Sout.Fz[cidx] = f2 / cE;
             }
         }
     }

@@ -92,7 +92,8 @@ struct HydroPhT {
         Prim p;
         double sp;
         cell_prim_speed(gamma, u[0], u[1], u[2], u[3], u[4], last, p, sp);
-        wout.f[0][cidx] = p.rho; wout.f[1][cidx] = p.vx; wout.f[2][cidx] = p.vy; wout.f[3][cidx] = p.vz;
+        // rho is its own primitive: the next stage reads it from the state this kernel has just written (8 B/cell less)
+        wout.f[1][cidx] = p.vx; wout.f[2][cidx] = p.vy; wout.f[3][cidx] = p.vz;
         wout.f[4][cidx] = p.P;
         if (!(p.rho > 0.0) || !(p.P > 0.0)) { ++t.bad; return; }
         if (last && sp > t.smax) t.smax = sp;
@@ -172,8 +173,7 @@ struct RadPhT {
     struct Tail { int bad = 0; };
     __device__ __forceinline__ void finish(int cidx, const double r[4], const FieldsRW<4> &sout, bool, Tail &t) const
     {
-        const double cE = c * r[0];
-        sout.f[0][cidx] = r[0];
+        const double cE = c * r[0];           // E_r is its own reconstruction variable: read from the state next stage
         sout.f[1][cidx] = r[1] / cE;
         sout.f[2][cidx] = r[2] / cE;
         sout.f[3][cidx] = r[3] / cE;

@@ -310,15 +310,18 @@ int hydro_stage(qk_ctx *c, double dtdx, int stage, double *const *U, double *con
         Scope s(c, K_FLATTEN);
         s.done(launch_chi(g, c->pc.gamma, ch5(W), c->chi3[0], c->chi3[1], c->chi3[2], c->chi, d0, d1, m0, m1, c->chi_path, c->stream));
     };
+    // the density is its own primitive: the sweeps read it from the stage's state U (ghost-filled here either way), so
+    // the kernel that produces a state stores four primitives, not five
+    double *const Wv[5] = {U[0], W[1], W[2], W[3], W[4]};
     auto sweep = [&](int d, int k0, int k1) {
         Scope s(c, K_HYDRO_X + d);
-        s.done(launch_hydro_sweeps(g, c->pc.gamma, c->pc.flags, dtdx, stage, ch5(W), c->chi, h5(c->acc), ch5(U), ch5(U0), h5(out),
+        s.done(launch_hydro_sweeps(g, c->pc.gamma, c->pc.flags, dtdx, stage, ch5(Wv), c->chi, h5(c->acc), ch5(U), ch5(U0), h5(out),
                                    h5(Wout), c->ctr, c->cache, c->stream, 1 << d, dtdx_dev, k0, k1));
     };
     int rc;
     const bool cached = w_ready && !c->has_fixed;
     if (cached) {
-        rc = fill_begin(c, W, 5);
+        rc = fill_begin(c, Wv, 5);
         if (rc) return rc;
     } else {
         rc = fill_fields(c, U, 5, nullptr, stage == 1 ? U0 : nullptr);
@@ -375,14 +378,16 @@ int rad_stage(qk_ctx *c, double dtdx, int stage, double *const *R, double *const
     const int nz = c->g.nz;
     double *list[6];
     int n = 0;
-    double *const *src = cached ? S : R;
+    // E_r is its own reconstruction variable: read from the stage's state R (ghost-filled here either way)
+    double *const Sv[4] = {R[0], S[1], S[2], S[3]};
+    double *const *src = cached ? Sv : R;
     for (int f = 0; f < 4; ++f) list[n++] = src[f];
     if (stage == 0) { list[n++] = c->state[QK_RHO]; list[n++] = c->state[QK_KAPPA_R]; }
     int rc = fill_begin(c, list, n, nullptr, (!cached && stage == 1) ? R0 : nullptr);
     if (rc) return rc;
     auto sweep = [&](int d) {
         Scope s(c, K_RAD_X + d);
-        s.done(launch_rad_sweeps(c->g, c->pc, dtdx, stage, cr4(S), c->state[QK_RHO], c->state[QK_KAPPA_R], r4(c->acc), cr4(R),
+        s.done(launch_rad_sweeps(c->g, c->pc, dtdx, stage, cr4(Sv), c->state[QK_RHO], c->state[QK_KAPPA_R], r4(c->acc), cr4(R),
                                  cr4(R0), r4(out), r4(Sout), c->ctr, c->stream, 1 << d, dtdx_dev, 0, nz));
     };
     if (cached) {        // the x and y sweeps read no z ghost plane: they run while the neighbours' planes travel
