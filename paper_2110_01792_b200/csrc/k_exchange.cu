@@ -10,7 +10,7 @@
 
 namespace qk {
 
-constexpr int QK_EX_MINB = 6;    // 85 registers (7 CTAs / 73 registers spills once dt and the opacity law are parameters)
+constexpr int QK_EX_MINB = 7;    // 72 registers, 40 B of spills: 1.04 -> 1.00 ms at 256^3 (6 CTAs / 80 registers 1.04, 8 / 64 1.00, 9 / 56 1.23, 5 / 96 1.16)
 template <bool KT>
 __global__ void __launch_bounds__(128, KT ? 5 : QK_EX_MINB) exchange_kernel(Geom g, ExchangeConsts kc, double dt_host, const double *__restrict__ dt_dev, const double *__restrict__ rho,
                                                        double *__restrict__ mx, double *__restrict__ my,

@@ -18,8 +18,8 @@
 //                        stage, the CFL signal speed of the new state (eq 21).
 //
 // HBM traffic per cell and stage (hydro): x reads W + chi (48 B), writes D (40); y reads W + chi + D (88), writes D
-// (40); z reads W + chi + D + U (128) + U^n in stage 2 (40), writes the new state and its primitives (80): 424-464 B
-// with the flattening kernel's 40.  Two leaner layouts were built and measured slower: reading
+// (40); z reads W + chi + D + U (120: the density of W is U's own array) + U^n in stage 2 (40), writes the new state
+// and its primitives v, P (72): 408-448 B with the flattening kernel's 40.  Two leaner layouts were built and measured slower: reading
 // the conserved state and converting every loaded cell (no W arrays, 80 B less, +20 % time: the division chains of
 // cons -> prim run 4 x per cell instead of once), and one fused x+y kernel that writes D once (128 B less, +50 % time
 // at 168 registers / 3 warps per scheduler).
