@@ -1,5 +1,8 @@
 """Pins for the hydro part of the CPU oracle (oracle/hydro.c): what the paper and the
 mathematics fix, not the oracle's own formulas.  CPU only."""
+import glob
+import hashlib
+import json
 import os
 
 import numpy as np
@@ -18,6 +21,37 @@ def _golden(name):
         if line and not line.startswith("#"):
             rows.append([float(x) for x in line.split()])
     return rows
+
+
+# ---- the two long pins (PAPER.md:299 at N = 1024): minutes each, because the oracle carries the full
+# ghost shell around an N x 1 x 1 box.  Their values depend on nothing but the oracle's sources and this file, so
+# tests/golden/make_oracle_slow_pins.py (which calls only the functions below, i.e. only oracle/) stores them next to a
+# SHA-256 of exactly those files; the tests take the stored value when the fingerprint still matches and compute it
+# otherwise (any change of the oracle, of its build flags or of this file) or when QK_SLOW=1.  Either way the assertion
+# against the paper's printed number runs.
+def _oracle_fingerprint():
+    root = os.path.dirname(HERE)
+    files = sorted(glob.glob(os.path.join(root, "oracle", "*.c")) + glob.glob(os.path.join(root, "oracle", "*.h")))
+    files += [os.path.join(root, "oracle", "__init__.py"), os.path.abspath(__file__)]
+    h = hashlib.sha256()
+    for f in files:
+        h.update(os.path.basename(f).encode())
+        h.update(open(f, "rb").read())
+    return h.hexdigest()
+
+
+SLOW_PINS = os.path.join(HERE, "golden", "oracle_slow_pins.json")
+
+
+def _slow_pin(name, compute):
+    if os.environ.get("QK_SLOW") != "1":
+        try:
+            stored = json.load(open(SLOW_PINS))
+            if stored["fingerprint"] == _oracle_fingerprint():
+                return float(stored["values"][name])
+        except (OSError, KeyError, ValueError):
+            pass
+    return compute()
 
 
 def _run_1d(N, prim_fn, gamma, t_end, cfl, bc=O.BC_PERIODIC, length=1.0, x0=0.0):
@@ -69,7 +103,7 @@ def test_sound_wave_printed_errors(row):
 
 
 def test_sound_wave_printed_error_1024():
-    e = _sound_wave_error(1024)
+    e = _slow_pin("sound_wave_error_1024", lambda: _sound_wave_error(1024))
     assert abs(e / 1.7e-11 - 1.0) < 0.05, e
 
 
@@ -169,9 +203,7 @@ def test_sod_against_exact_solution():
     assert 1.6 < errs[0] / errs[1] < 2.6 and 1.6 < errs[1] / errs[2] < 2.6, errs
 
 
-def test_strong_shock_tube_error_scale():
-    """PAPER.md:313-315: (rho,p) = (10,100)|(1,1), 1000 cells on [0,5], x0=2, t=0.4, CFL 0.1;
-    relative rms-of-L1 error printed as 1.12e-3 (gamma not printed; 1.4 assumed: weak pin, ~1e-3)."""
+def _strong_shock_rel_error():
     def ic(x):
         return np.where(x < 2.0, 10.0, 1.0), 0 * x, np.where(x < 2.0, 100.0, 1.0)
     g = 1.4
@@ -180,9 +212,16 @@ def test_strong_shock_tube_error_scale():
     Uex = [r, r * u, p / (g - 1) + 0.5 * r * u * u]
     num = np.sqrt(np.mean([np.abs(U[k] - Uex[n]).mean() ** 2 for n, k in enumerate((0, 1, 4))]))
     den = np.sqrt(np.mean([np.abs(Uex[n]).mean() ** 2 for n in range(3)]))
+    return float(num / den)
+
+
+def test_strong_shock_tube_error_scale():
+    """PAPER.md:313-315: (rho,p) = (10,100)|(1,1), 1000 cells on [0,5], x0=2, t=0.4, CFL 0.1;
+    relative rms-of-L1 error printed as 1.12e-3 (gamma not printed; 1.4 assumed: weak pin, ~1e-3)."""
+    rel = _slow_pin("strong_shock_rel_error", _strong_shock_rel_error)
     # paper: 1.12e-3 (gamma = 1.4 gives 1.19e-3 here, gamma = 5/3 1.31e-3); within 20 % of the printed value -- without
     # flattening the paper reports "unacceptably large post-shock oscillations", so this holds the H6 constants to scale
-    assert 0.9e-3 < num / den < 1.35e-3, num / den
+    assert 0.9e-3 < rel < 1.35e-3, rel
 
 
 SLOW_SHOCK = dict(gamma=1.4, L=(3.86, -3.1266, 27.0913), R=(1.0, -3.44, 8.4168), speed=0.1096)     # PAPER.md:357-366
